@@ -1,0 +1,147 @@
+/*
+ * include/ccake.h — C ABI of libccake: the B200-native (sm_100a) SPH hot path of CCAKE 2.0.
+ *
+ * The library advances the SPH state  phi_a = { r^i, u^i, S = s/sigma, N_q = n_q/sigma, Pi/sigma, pi^{ij}/sigma,
+ * J^i_q/sigma }  (Eq. 85 :954) of all particles by explicit Runge-Kutta steps of  d phi_a / dx0
+ * (Eq. 87 :964).  One RK substep runs, in this order and entirely in CUDA kernels on the context's stream
+ * (DESIGN.md §"Kernels"):
+ *   a1 bounding box, a2 cell hash, a3 stable radix sort by cell + cell lists      (PAPER.md :1434, §5.9.1)
+ *   a4 smoothing sums sigma*, s*, rho*_B, rho*_S, rho*_Q                          (Eq. 71-72 :877-882, Eq. 77 :910)
+ *   a5 rest-frame densities (Eq. 68 :864), equation of state: 4-D table gather by quadrilinear interpolation
+ *      (:583-593) or the closed-form conformal family (App. A :2115-2156), transport coefficients (§5.3)
+ *   a6 pairwise gradient sums with dW_ab (Eq. 79 :920, Eq. 81-82 :934-938)
+ *   a7 per-particle equations of motion reduced to a D x D solve (Eq. 87-104 :964-1041, Eq. 95 :988)
+ *   a8 RK stage update;  a9 conserved totals (§5.6.5 :1049-1063) on request.
+ *
+ * Units: fm (hbar = c = 1): T, mu in fm^-1; s, n_q in fm^-3; e, p in fm^-4.  All arithmetic is fp64.
+ *
+ * Conventions common to every call
+ *   - Returns CCAKE_OK (0) or a negative CCAKE_E* code; never throws, aborts or prints.  Text of the last error
+ *     of a context: ccake_last_error().
+ *   - Ownership: the caller owns every buffer it passes; the library copies on load and writes into caller
+ *     buffers on read.  The context owns its device memory until ccake_destroy().
+ *   - `memspace`: CCAKE_HOST (0) = host pointers, CCAKE_DEVICE (1) = device pointers on the context's device
+ *     (e.g. torch.Tensor.data_ptr()).  Pointer ARRAYS (cols, axes, field_ids) are always host arrays.
+ *   - Work is enqueued on the context's stream.  ccake_step() is asynchronous; calls that return data to the
+ *     host synchronise the stream before returning.  One context per host thread.
+ *   - There is no CPU fallback: without a usable CUDA device ccake_create() fails with CCAKE_ECUDA.
+ */
+#ifndef CCAKE_H
+#define CCAKE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { CCAKE_OK = 0, CCAKE_EINVAL = -1, CCAKE_ENOMEM = -2, CCAKE_ECUDA = -3, CCAKE_ESTATE = -4, CCAKE_ERANGE = -5 };
+enum { CCAKE_HOST = 0, CCAKE_DEVICE = 1 };
+
+/* Field ids.  State fields can be loaded and read; derived fields are read-only and are evaluated at the
+ * current state (one evaluation of steps a1-a7 without an update). */
+enum {
+  CCAKE_R1 = 0, CCAKE_R2, CCAKE_R3,           /* position r^i (x, y, z | eta_s)                                */
+  CCAKE_U1, CCAKE_U2, CCAKE_U3,               /* contravariant u^i; u^0 = gamma follows from u.u = 1           */
+  CCAKE_S, CCAKE_NB, CCAKE_NS, CCAKE_NQ,      /* S = s/sigma, N_q = n_q/sigma (Eq. 84-86)                      */
+  CCAKE_BULK,                                 /* Pi/sigma                                                      */
+  CCAKE_PI11, CCAKE_PI12, CCAKE_PI13, CCAKE_PI22, CCAKE_PI23, CCAKE_PI33,   /* pi^{ij}/sigma                  */
+  CCAKE_JB1, CCAKE_JB2, CCAKE_JB3, CCAKE_JS1, CCAKE_JS2, CCAKE_JS3, CCAKE_JQ1, CCAKE_JQ2, CCAKE_JQ3, /* J^i_q/sigma */
+  CCAKE_MASS = 26,                            /* SPH weight m_b (default 1, Eq. 75 :898)                       */
+  CCAKE_WORK = 27,                            /* accumulated longitudinal work (2+1D hyperbolic), starts at 0  */
+  CCAKE_NSTATE = 28,
+  CCAKE_SIGMA_STAR = 32, CCAKE_S_DENS, CCAKE_RHO_B, CCAKE_RHO_S, CCAKE_RHO_Q,  /* sigma*, rest-frame s, n_q   */
+  CCAKE_T, CCAKE_MU_B, CCAKE_MU_S, CCAKE_MU_Q,
+  CCAKE_P = 41, CCAKE_E, CCAKE_CS2, CCAKE_GAMMA, CCAKE_NNB, CCAKE_CELL, CCAKE_THETA, CCAKE_SIGMA, CCAKE_S_STAR,
+  CCAKE_RHOSTAR_B = 50, CCAKE_RHOSTAR_S, CCAKE_RHOSTAR_Q, CCAKE_WS, CCAKE_DIVV,
+  CCAKE_FM1 = 55, CCAKE_FM2, CCAKE_FM3,       /* right-hand side of the momentum equation, sqrt(-g)(FP_i - FB_i) */
+  CCAKE_FK_B = 58, CCAKE_FK_S, CCAKE_FK_Q,    /* right-hand side of the charge equation, -sqrt(-g) FK_q         */
+  CCAKE_RATE = 64                             /* CCAKE_RATE + state id: d(state field)/dx0 at the current state */
+};
+
+/* EoS table column ids (ccake_load_eos_table): T, mu_B, mu_S, mu_Q, p, c_s^2, e, dw/ds|_n, dw/dn_B, dw/dn_S, dw/dn_Q */
+enum {
+  CCAKE_COL_T = 0, CCAKE_COL_MUB, CCAKE_COL_MUS, CCAKE_COL_MUQ, CCAKE_COL_P, CCAKE_COL_CS2, CCAKE_COL_E,
+  CCAKE_COL_WS, CCAKE_COL_WB, CCAKE_COL_WSQ, CCAKE_COL_WQ, CCAKE_NCOLS_MAX
+};
+
+/* Plain data, copied by ccake_create(). */
+typedef struct ccake_params {
+  int32_t dim;         /* 2 | 3 evolved spatial dimensions                                               */
+  int32_t coords;      /* 0 Cartesian (t,x,y,z) | 1 hyperbolic (tau,x,y,eta_s), PAPER.md :488            */
+  int32_t integrator;  /* 2 RK2 midpoint | 4 classical RK4 (the paper names no scheme; DESIGN reading 7) */
+  int32_t eom;         /* 0 ideal | 1 Israel-Stewart minimal (Eq. 49-51 :676-680) | 2 DNMR shear+bulk (Eq. 52) */
+  int32_t flags;       /* bit0 shear, bit1 bulk, bit2 BSQ diffusion (ignored when eom == 0)              */
+  int32_t eos_kind;    /* 0 closed-form conformal p = c0 T^4 + c2 T^2 sum mu^2 + c4 sum mu^4 | 1 table   */
+  int32_t device;      /* CUDA device ordinal                                                            */
+  int32_t reserved0;
+  void*   stream;      /* cudaStream_t to enqueue on, or NULL for the default stream                     */
+  double  h;           /* smoothing length, support 2h (Eq. 77)                                          */
+  double  x0_start;    /* initial time t or tau (> 0 for hyperbolic)                                     */
+  double  dx0;         /* step size of one full RK step                                                  */
+  double  eos_c0, eos_c2, eos_c4;
+  double  eta_over_s, tau_pi_coeff, tau_floor;              /* tau_pi = max(coeff * eta / w, floor)      */
+  double  zeta_max, zeta_T_peak, zeta_width, tau_Pi_coeff;  /* zeta/s = zeta_max W^2/(W^2 + (T-T_peak)^2) or
+                                                               constant zeta_max when zeta_width <= 0;
+                                                               tau_Pi = tau_Pi_coeff * tau_pi              */
+  double  kappa_over_T2[9];   /* row-major 3x3 kappa_qq'/T^2 (:769, :779)                                */
+  double  tau_q_times_T[3];   /* tau_q T (:781)                                                           */
+  double  dnmr_coeffs[8];     /* delta_PiPi/tau_Pi, lambda_Pipi/tau_Pi, delta_pipi/tau_pi, tau_pipi/tau_pi,
+                                 lambda_piPi, phi_omega (coefficient of the vorticity term), 2 unused     */
+} ccake_params;
+
+typedef struct ccake_ctx ccake_ctx;   /* opaque; owns all device memory */
+
+/* Create a context on params->device.  EINVAL for out-of-range parameters, ECUDA when the device or the
+ * kernels (sm_100a) are unusable. */
+int ccake_create(const ccake_params* p, ccake_ctx** out);
+int ccake_destroy(ccake_ctx* c);
+
+/* Load n particles.  cols[k] (n doubles, `memspace`) holds state field field_ids[k]; fields not given are 0
+ * (MASS: 1).  Fields of switched-off sectors (and the third components when dim == 2) are ignored.  Resets the
+ * time to x0_start.  Particle index = position in these arrays ("original order"). */
+int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* field_ids,
+                         const double* const* cols, int32_t memspace);
+
+/* Load the offline-inverted EoS table (PAPER.md :583-593).  Axis 0 is s; axes 1..3 are B, S, Q, each either the
+ * density n_q (axis_kind 0) or the ratio n_q / s (axis_kind 1).  axes[k] = dims[k] strictly increasing node
+ * values (any spacing, e.g. the paper's log-decade pattern).  data is row-major [d0][d1][d2][d3][ncols] with
+ * column k holding quantity col_ids[k]; columns T..WS are required, WB..WQ when diffusion is on.  Lookup is
+ * quadrilinear; coordinates outside the table are clamped and counted (totals[11]). */
+int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4],
+                         const double* const axes[4], int32_t ncols, const int32_t* col_ids,
+                         const double* data, int32_t memspace);
+
+/* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
+int ccake_step(ccake_ctx* c, int32_t nsteps);
+
+/* Wait for the stream.  ERANGE when, since the last load, a particle left the EoS table, a per-particle solve
+ * was singular or a field became NaN (the state stays readable); ECUDA on a device fault. */
+int ccake_synchronize(ccake_ctx* c);
+
+/* Read fields in ORIGINAL particle order into cols[k] (capacity doubles each, capacity >= n). */
+int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* field_ids, double* const* cols,
+                      int64_t capacity, int32_t memspace);
+
+/* out (host) = { x0, E, P_1, P_2, P_3, S_tot, N_B, N_S, N_Q, sum m, work, n_out_of_table, max |trace pi|,
+ *                n_bad, sum_a N_nb(a), 0 } at the current state (DESIGN.md §"Totals"). */
+int ccake_conserved_totals(ccake_ctx* c, double out[16]);
+
+/* Test hook: neighbour sets {b != a : r_ab^2 < (2h)^2} of the current state, ORIGINAL indices, ascending per
+ * particle, CSR.  counts (n), offsets (n+1, may be NULL), list (cap entries, may be NULL to query counts);
+ * all host pointers. */
+int ccake_read_neighbors(ccake_ctx* c, int64_t* counts, int64_t* offsets, int32_t* list, int64_t cap);
+
+/* Test hook for sizes where lists do not fit: per particle (original order) the order-free hash
+ * sum_b mix64(b) mod 2^64 over its neighbour set, mix64 = the splitmix64 finaliser of (b + 1).  Host pointer. */
+int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity);
+
+/* Measurement hook: average device time in ms of each kernel group over the substeps run since the last
+ * call (out[0..7] = bbox+hash+sort, pack, smoothing, thermo/EoS, gradient, EoM+update, totals, substeps). */
+int ccake_kernel_times(ccake_ctx* c, double out[8]);
+int ccake_enable_timing(ccake_ctx* c, int32_t on);
+
+const char* ccake_last_error(const ccake_ctx* c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

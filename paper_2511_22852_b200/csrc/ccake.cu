@@ -1,0 +1,839 @@
+/*
+ * csrc/ccake.cu — libccake: C ABI (include/ccake.h), context, device memory and the stream-ordered step driver.
+ * Every step of the hot path runs in the CUDA kernels of this directory; the host code below only allocates,
+ * marshals and launches.  There is no CPU fallback.
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "eom.cuh"
+#include "grid_sort.cuh"
+#include "pair_tiled.cuh"
+#include "pair_v1.cuh"
+#include "thermo_eos.cuh"
+#include "totals.cuh"
+
+using namespace ccake;
+
+namespace {
+enum { TG_SORT = 0, TG_PACK, TG_SMOOTH, TG_THERMO, TG_GRAD, TG_EOM, TG_TOTALS, TG_N };
+}
+
+struct ccake_ctx {
+  ccake_params P;
+  KParams kp;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int64_t N = 0, npad = 0;
+  bool loaded = false, table_loaded = false, derived_valid = false;
+  double x0 = 0.0;
+  uint32_t field_mask = 0;
+  int pair_impl = 0;    /* 0 tiled kernels, 1 thread-per-particle v1 */
+
+  double* Y[3] = {nullptr, nullptr, nullptr};   /* Y0, stage, RK4 accumulator */
+  double* Krate = nullptr;
+  uint32_t* orig[2] = {nullptr, nullptr};
+  uint32_t *key[2] = {nullptr, nullptr}, *val[2] = {nullptr, nullptr};
+  uint32_t *hist = nullptr, *chunk_tot = nullptr, *cell_start = nullptr;
+  int ntiles = 0, passes = 1, max_cells = 1 << 8;
+  int64_t hist_len = 0;
+  int nchunks = 0;
+  Grid* grid = nullptr;
+  Status* status = nullptr;
+  double* bbox_partial = nullptr;
+  int bbox_blocks = 0;
+  double *tot_partial = nullptr, *tot_out = nullptr;
+  int tot_blocks = 0;
+  double* arena = nullptr;      /* sorted-order doubles */
+  uint32_t* nnb = nullptr;
+  double* theta = nullptr;
+  double* scratch = nullptr;    /* N doubles: read_fields staging */
+  Sorted so;
+  PairWork pw;
+
+  TableDev tb;
+  double* tb_axes = nullptr;
+  double* tb_data = nullptr;
+
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;
+  size_t ev_used = 0;
+  int64_t substeps_timed = 0;
+
+  std::string err;
+};
+
+namespace {
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                                 \
+      return (e_ == cudaErrorMemoryAllocation) ? CCAKE_ENOMEM : CCAKE_ECUDA;                        \
+    }                                                                                              \
+  } while (0)
+
+inline int nblk(int64_t n, int t) { return (int)((n + t - 1) / t); }
+
+void free_particles(ccake_ctx* c) {
+  for (int k = 0; k < 3; ++k) { cudaFree(c->Y[k]); c->Y[k] = nullptr; }
+  cudaFree(c->Krate); c->Krate = nullptr;
+  for (int k = 0; k < 2; ++k) {
+    cudaFree(c->orig[k]); c->orig[k] = nullptr;
+    cudaFree(c->key[k]); c->key[k] = nullptr;
+    cudaFree(c->val[k]); c->val[k] = nullptr;
+  }
+  cudaFree(c->hist); c->hist = nullptr;
+  cudaFree(c->chunk_tot); c->chunk_tot = nullptr;
+  cudaFree(c->cell_start); c->cell_start = nullptr;
+  cudaFree(c->bbox_partial); c->bbox_partial = nullptr;
+  cudaFree(c->tot_partial); c->tot_partial = nullptr;
+  cudaFree(c->tot_out); c->tot_out = nullptr;
+  cudaFree(c->arena); c->arena = nullptr;
+  cudaFree(c->nnb); c->nnb = nullptr;
+  cudaFree(c->theta); c->theta = nullptr;
+  cudaFree(c->scratch); c->scratch = nullptr;
+  pair_work_free(c->pw);
+  c->loaded = false;
+}
+
+void free_table(ccake_ctx* c) {
+  cudaFree(c->tb_axes); c->tb_axes = nullptr;
+  cudaFree(c->tb_data); c->tb_data = nullptr;
+  c->table_loaded = false;
+}
+
+int mark(ccake_ctx* c) {
+  if (!c->timing) return CCAKE_OK;
+  if (c->ev_used == c->ev.size()) {
+    cudaEvent_t e;
+    CK(cudaEventCreate(&e));
+    c->ev.push_back(e);
+  }
+  CK(cudaEventRecord(c->ev[c->ev_used++], c->stream));
+  return CCAKE_OK;
+}
+
+/* layout of the sorted-order arena */
+constexpr int ARENA_FIELDS = 3 + 1 + 3 + 1 + 5 + 6 + 11 + 1 + 9 + 9 + 3 + 3 + 3 + 3 + 3 + 3 + 9 + 9 + 1;
+
+void carve(ccake_ctx* c) {
+  Sorted& s = c->so;
+  double* p = c->arena;
+  const int64_t np = c->npad;
+  auto take = [&]() { double* r = p; p += np; return r; };
+  for (int k = 0; k < 3; ++k) s.x[k] = take();
+  s.S = take();
+  for (int q = 0; q < NQ; ++q) s.Nq[q] = take();
+  s.m = take();
+  s.sigma_star = take(); s.s_star = take();
+  for (int q = 0; q < NQ; ++q) s.rho_star[q] = take();
+  s.gamma = take(); s.sigma = take(); s.s = take();
+  for (int q = 0; q < NQ; ++q) s.n[q] = take();
+  s.T = take();
+  for (int q = 0; q < NQ; ++q) s.mu[q] = take();
+  s.p = take(); s.e = take(); s.cs2 = take(); s.ws = take();
+  for (int q = 0; q < NQ; ++q) s.wq[q] = take();
+  s.Ppair = take();
+  for (int k = 0; k < 9; ++k) s.Bpair[k] = take();
+  for (int k = 0; k < 9; ++k) s.Kpair[k] = take();
+  for (int q = 0; q < NQ; ++q) s.alpha[q] = take();
+  for (int k = 0; k < 3; ++k) s.v[k] = take();
+  for (int k = 0; k < 3; ++k) s.u[k] = take();
+  for (int k = 0; k < 3; ++k) s.FP[k] = take();
+  for (int k = 0; k < 3; ++k) s.FB[k] = take();
+  for (int q = 0; q < NQ; ++q) s.FK[q] = take();
+  for (int k = 0; k < 9; ++k) s.DU[k] = take();
+  for (int k = 0; k < 9; ++k) s.DA[k] = take();
+  s.divv = take();
+  s.nnb = c->nnb;
+  s.cell_start = c->cell_start;
+}
+
+int launch_check(ccake_ctx* c, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return CCAKE_ECUDA;
+  }
+  return CCAKE_OK;
+}
+
+/* steps a1-a3 on the state Ycur; optionally reorder the store physically (then perm = identity) */
+int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
+  const int64_t N = c->N, np = c->npad;
+  const int D = c->P.dim;
+  cudaStream_t st = c->stream;
+  bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, st>>>(Ycur, np, N, D, c->bbox_partial);
+  bbox_final_kernel<<<1, 32, 0, st>>>(c->bbox_partial, c->bbox_blocks, D, c->P.h, c->max_cells, c->grid);
+  cell_hash_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->grid, c->key[0], c->val[0]);
+  int cur = 0;
+  for (int pass = 0; pass < c->passes; ++pass) {
+    const int shift = 8 * pass;
+    radix_hist_kernel<<<c->ntiles, SORT_THREADS, 0, st>>>(c->key[cur], N, shift, c->ntiles, c->hist);
+    scan_chunk_kernel<<<c->nchunks, SCAN_CHUNK, 0, st>>>(c->hist, c->hist_len, c->chunk_tot);
+    scan_totals_kernel<<<1, 1024, 0, st>>>(c->chunk_tot, c->nchunks);
+    radix_scatter_kernel<<<c->ntiles, SORT_THREADS, 0, st>>>(c->key[cur], c->val[cur], N, shift, c->ntiles, c->hist,
+                                                              c->chunk_tot, c->key[cur ^ 1], c->val[cur ^ 1]);
+    cur ^= 1;
+  }
+  c->so.key = c->key[cur];
+  c->so.perm = c->val[cur];
+  cell_start_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.key, N, c->grid, c->cell_start);
+  if (reorder) {
+    /* Ycur must be Y[0]; Y[1] is free at the first substep of a step */
+    reorder_store_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], c->Y[1], np, N, c->so.perm, c->field_mask | (1u << CCAKE_MASS),
+                                                        c->orig[0], c->orig[1]);
+    std::swap(c->Y[0], c->Y[1]);
+    std::swap(c->orig[0], c->orig[1]);
+    Ycur = c->Y[0];
+    iota_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.perm, N);
+  }
+  return launch_check(c, "build_cells");
+}
+
+template <int D>
+int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
+  const int64_t N = c->N, np = c->npad;
+  cudaStream_t st = c->stream;
+  const KParams& kp = c->kp;
+  const Geom gm = make_geom(c->P.coords, x0s);
+  int rc;
+  pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->so);
+  if ((rc = mark(c))) return rc;
+  /* a4 */
+  if (c->pair_impl == 1) smoothing_v1_kernel<D><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
+  else if ((rc = launch_smoothing_tiled<D>(c->pw, N, kp, c->grid, c->so, st))) { c->err = "smoothing launch"; return CCAKE_ECUDA; }
+  if ((rc = mark(c))) return rc;
+  /* a5 */
+  cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
+  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, c->tb, Ycur, np, c->so, c->status);
+  if ((rc = mark(c))) return rc;
+  /* a6 */
+  const bool visc = kp.shear, diff = kp.diff;
+  if (c->pair_impl == 1) {
+    if (visc && diff) gradient_v1_kernel<D, true, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
+    else if (visc) gradient_v1_kernel<D, true, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
+    else if (diff) gradient_v1_kernel<D, false, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
+    else gradient_v1_kernel<D, false, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
+  } else if ((rc = launch_gradient_tiled<D>(c->pw, N, kp, c->grid, c->so, visc, diff, st))) { c->err = "gradient launch"; return CCAKE_ECUDA; }
+  if ((rc = mark(c))) return rc;
+  /* a7 + a8 */
+  RkArgs rk = rk_in;
+  rk.Ycur = Ycur;
+  rk.theta_out = c->theta;
+  eom_kernel<D><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
+  if ((rc = mark(c))) return rc;
+  return launch_check(c, "substep");
+}
+
+int substep(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk) {
+  int rc;
+  if ((rc = mark(c))) return rc;
+  if ((rc = build_cells(c, Ycur, false))) return rc;
+  if ((rc = mark(c))) return rc;
+  if (c->P.dim == 2) rc = pair_and_eom<2>(c, Ycur, x0s, rk);
+  else rc = pair_and_eom<3>(c, Ycur, x0s, rk);
+  if (c->timing) c->substeps_timed++;
+  return rc;
+}
+
+int rk_step(ccake_ctx* c) {
+  const double dt = c->P.dx0, x0 = c->x0;
+  int rc;
+  RkArgs rk;
+  std::memset(&rk, 0, sizeof(rk));
+  rk.update = 1;
+  if (c->P.integrator == 2) {
+    /* midpoint (DESIGN reading 7): k1 = f(y0, x0); yh = y0 + dt/2 k1; k2 = f(yh, x0 + dt/2); y1 = y0 + dt k2.
+       The first substep reorders Y[0] into Y[1] and swaps, so "base" and "out" are named after the swap. */
+    rk.acc_mode = 0;
+    rk.c_out = 0.5 * dt;
+    rk.Ybase = nullptr; rk.Yout = nullptr;
+    {
+      double* Ycur = c->Y[0];
+      if ((rc = mark(c))) return rc;
+      if ((rc = build_cells(c, Ycur, true))) return rc;
+      if ((rc = mark(c))) return rc;
+      rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
+      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, x0, rk) : pair_and_eom<3>(c, Ycur, x0, rk);
+      if (rc) return rc;
+      if (c->timing) c->substeps_timed++;
+    }
+    rk.c_out = dt; rk.Ybase = c->Y[0]; rk.Yout = c->Y[0];
+    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+  } else {
+    rk.Yacc = c->Y[2];
+    {
+      double* Ycur = c->Y[0];
+      if ((rc = mark(c))) return rc;
+      if ((rc = build_cells(c, Ycur, true))) return rc;
+      if ((rc = mark(c))) return rc;
+      rk.Ybase = c->Y[0]; rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt; rk.acc_mode = 1; rk.w_acc = 1.0;
+      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, x0, rk) : pair_and_eom<3>(c, Ycur, x0, rk);
+      if (rc) return rc;
+      if (c->timing) c->substeps_timed++;
+    }
+    rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
+    rk.c_out = 0.5 * dt; rk.acc_mode = 2; rk.w_acc = 2.0;
+    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+    rk.c_out = dt;
+    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+    rk.Yout = c->Y[0]; rk.c_out = dt / 6.0; rk.acc_mode = 3;
+    if ((rc = substep(c, c->Y[1], x0 + dt, rk))) return rc;
+  }
+  c->x0 = x0 + dt;
+  c->derived_valid = false;
+  return CCAKE_OK;
+}
+
+/* evaluate a1-a7 at the current state without an update (derived fields, rates, totals) */
+int refresh(ccake_ctx* c) {
+  if (c->derived_valid) return CCAKE_OK;
+  if (!c->Krate) {
+    CK(cudaMalloc(&c->Krate, sizeof(double) * c->npad * NSTATE));
+  }
+  CK(cudaMemsetAsync(c->Krate, 0, sizeof(double) * c->npad * NSTATE, c->stream));
+  const bool t = c->timing;
+  c->timing = false;
+  RkArgs rk;
+  std::memset(&rk, 0, sizeof(rk));
+  rk.update = 0;
+  rk.Krate = c->Krate;
+  double* Ycur = c->Y[0];
+  int rc = build_cells(c, Ycur, true);
+  if (!rc) {
+    rk.Ybase = c->Y[0]; rk.Yout = c->Y[0];
+    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, c->x0, rk) : pair_and_eom<3>(c, Ycur, c->x0, rk);
+  }
+  c->timing = t;
+  if (rc) return rc;
+  c->derived_valid = true;
+  return CCAKE_OK;
+}
+
+__global__ void scatter_store_kernel(const double* __restrict__ src, const uint32_t* __restrict__ orig, int64_t n,
+                                     double* __restrict__ dst) {
+  const int64_t a = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (a < n) dst[orig[a]] = src[a];
+}
+__global__ void scatter_sorted_kernel(const double* __restrict__ src, const uint32_t* __restrict__ perm,
+                                      const uint32_t* __restrict__ orig, int64_t n, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[orig[perm[i]]] = src[i];
+}
+__global__ void scatter_sorted_u32_kernel(const uint32_t* __restrict__ src, const uint32_t* __restrict__ perm,
+                                          const uint32_t* __restrict__ orig, int64_t n, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[orig[perm[i]]] = (double)src[i];
+}
+__global__ void scatter_diff_kernel(const double* __restrict__ x, const double* __restrict__ y, double scale,
+                                    const uint32_t* __restrict__ perm, const uint32_t* __restrict__ orig, int64_t n,
+                                    double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[orig[perm[i]]] = scale * (x[i] - (y ? y[i] : 0.0));
+}
+__global__ void gather_load_kernel(const double* __restrict__ src, int64_t n, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = src[i];
+}
+__global__ void fill_kernel(double* __restrict__ dst, int64_t n, double v) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = v;
+}
+
+__device__ inline uint64_t mix64(uint64_t z) {
+  z += 0x9E3779B97F4A7C15ULL;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+
+/* walk the neighbour set of sorted slot i; mode 0: hash, mode 1: write original ids at list[offset..] */
+template <int D>
+__global__ void neighbour_walk_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
+                                      const uint32_t* __restrict__ orig, int mode, unsigned long long* __restrict__ hash_out,
+                                      const long long* __restrict__ offsets, int* __restrict__ list) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Grid g = *grid;
+  const uint32_t cid = so.key[i];
+  const int cx = cid % g.nc[0], cy = (cid / g.nc[0]) % g.nc[1], cz = cid / (g.nc[0] * g.nc[1]);
+  const double xa = so.x[0][i], ya = so.x[1][i], za = (D == 3) ? so.x[2][i] : 0.0;
+  const uint32_t ao = orig[so.perm[i]];
+  unsigned long long hsum = 0;
+  long long w = (mode == 1) ? offsets[ao] : 0;
+  const int z0 = (D == 3) ? -1 : 0, z1 = (D == 3) ? 1 : 0;
+  for (int dz = z0; dz <= z1; ++dz) {
+    const int zz = cz + dz;
+    if (zz < 0 || zz >= g.nc[2]) continue;
+    for (int dy = -1; dy <= 1; ++dy) {
+      const int yy = cy + dy;
+      if (yy < 0 || yy >= g.nc[1]) continue;
+      const int xlo = max(cx - 1, 0), xhi = min(cx + 1, g.nc[0] - 1);
+      const int row = g.nc[0] * (yy + g.nc[1] * zz);
+      const uint32_t b0 = so.cell_start[row + xlo], b1 = so.cell_start[row + xhi + 1];
+      for (uint32_t b = b0; b < b1; ++b) {
+        if (b == (uint32_t)i) continue;
+        const double r2 = dist2_exact(xa - so.x[0][b], ya - so.x[1][b], (D == 3) ? za - so.x[2][b] : 0.0, D);
+        if (r2 < kp.cut2) {
+          const uint32_t bo = orig[so.perm[b]];
+          if (mode == 0) hsum += mix64((uint64_t)bo + 1ULL);
+          else list[w++] = (int)bo;
+        }
+      }
+    }
+  }
+  if (mode == 0) hash_out[ao] = hsum;
+}
+
+}  // namespace
+
+/* ================================================================================================ C ABI ==== */
+extern "C" {
+
+const char* ccake_last_error(const ccake_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int ccake_create(const ccake_params* p, ccake_ctx** out) {
+  if (!p || !out) return CCAKE_EINVAL;
+  *out = nullptr;
+  if ((p->dim != 2 && p->dim != 3) || (p->coords != 0 && p->coords != 1) || (p->integrator != 2 && p->integrator != 4) ||
+      p->eom < 0 || p->eom > 2 || (p->eos_kind != 0 && p->eos_kind != 1) || !(p->h > 0.0) || !(p->dx0 > 0.0))
+    return CCAKE_EINVAL;
+  if (p->coords == 1 && !(p->x0_start > 0.0)) return CCAKE_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return CCAKE_ECUDA;   /* no CPU fallback */
+  if (p->device < 0 || p->device >= ndev) return CCAKE_EINVAL;
+  ccake_ctx* c = new (std::nothrow) ccake_ctx();
+  if (!c) return CCAKE_ENOMEM;
+  c->P = *p;
+  if (c->P.eom == 0) c->P.flags = 0;
+  c->device = p->device;
+  c->stream = (cudaStream_t)p->stream;
+  c->x0 = p->x0_start;
+  std::memset(&c->so, 0, sizeof(c->so));
+  std::memset(&c->tb, 0, sizeof(c->tb));
+  std::memset(&c->pw, 0, sizeof(c->pw));
+  if (cudaSetDevice(c->device) != cudaSuccess) { delete c; return CCAKE_ECUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess || prop.major < 10) {
+    /* kernels are built for sm_100a only */
+    delete c;
+    return CCAKE_ECUDA;
+  }
+  KParams& k = c->kp;
+  std::memset(&k, 0, sizeof(k));
+  k.D = p->dim; k.coords = p->coords; k.eom = p->eom; k.eos_kind = p->eos_kind;
+  k.shear = (c->P.eom != 0 && (c->P.flags & 1)) ? 1 : 0;
+  k.bulk = (c->P.eom != 0 && (c->P.flags & 2)) ? 1 : 0;
+  k.diff = (c->P.eom != 0 && (c->P.flags & 4)) ? 1 : 0;
+  k.h = p->h; k.inv_h = 1.0 / p->h;
+  { const double twoh = 2.0 * p->h; k.cut2 = twoh * twoh; }
+  const double pi = 3.14159265358979323846;
+  k.sigma_d = (p->dim == 2) ? 10.0 / (7.0 * pi * p->h * p->h) : 1.0 / (pi * p->h * p->h * p->h);
+  k.c0 = p->eos_c0; k.c2 = p->eos_c2; k.c4 = p->eos_c4;
+  k.eta_over_s = p->eta_over_s; k.tau_pi_coeff = p->tau_pi_coeff; k.tau_floor = p->tau_floor;
+  k.zeta_max = p->zeta_max; k.zeta_T_peak = p->zeta_T_peak; k.zeta_width = p->zeta_width; k.tau_Pi_coeff = p->tau_Pi_coeff;
+  for (int i = 0; i < 9; ++i) k.kappa_over_T2[i] = p->kappa_over_T2[i];
+  for (int i = 0; i < 3; ++i) k.tau_q_times_T[i] = p->tau_q_times_T[i];
+  for (int i = 0; i < 8; ++i) k.dnmr[i] = p->dnmr_coeffs[i];
+  /* active state fields */
+  uint32_t m = 0;
+  auto on = [&](int f) { m |= (1u << f); };
+  on(CCAKE_R1); on(CCAKE_R2); on(CCAKE_U1); on(CCAKE_U2);
+  if (p->dim == 3) { on(CCAKE_R3); on(CCAKE_U3); }
+  on(CCAKE_S); on(CCAKE_NB); on(CCAKE_NS); on(CCAKE_NQ);
+  if (k.bulk) on(CCAKE_BULK);
+  if (k.shear) {
+    on(CCAKE_PI11); on(CCAKE_PI12); on(CCAKE_PI22); on(CCAKE_PI33);
+    if (p->dim == 3) { on(CCAKE_PI13); on(CCAKE_PI23); }
+  }
+  if (k.diff)
+    for (int q = 0; q < 3; ++q) for (int j = 0; j < p->dim; ++j) on(CCAKE_JB1 + 3 * q + j);
+  if (p->coords == 1 && p->dim == 2) on(CCAKE_WORK);
+  c->field_mask = m;
+  const char* impl = std::getenv("CCAKE_PAIR_IMPL");
+  c->pair_impl = (impl && impl[0] == '1') ? 1 : 0;
+  if (cudaMalloc(&c->grid, sizeof(Grid)) != cudaSuccess || cudaMalloc(&c->status, sizeof(Status)) != cudaSuccess) {
+    cudaFree(c->grid);
+    delete c;
+    return CCAKE_ENOMEM;
+  }
+  cudaMemset(c->status, 0, sizeof(Status));
+  *out = c;
+  return CCAKE_OK;
+}
+
+int ccake_destroy(ccake_ctx* c) {
+  if (!c) return CCAKE_OK;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  free_particles(c);
+  free_table(c);
+  cudaFree(c->grid);
+  cudaFree(c->status);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  delete c;
+  return CCAKE_OK;
+}
+
+int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* ids, const double* const* cols,
+                         int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (n <= 0 || nfields <= 0 || !ids || !cols || n > 2000000000LL || (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_load_particles";
+    return CCAKE_EINVAL;
+  }
+  for (int k = 0; k < nfields; ++k)
+    if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in load"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  free_particles(c);
+  c->N = n;
+  c->npad = (n + 31) / 32 * 32;
+  const int64_t np = c->npad;
+  const int nbuf = (c->P.integrator == 4) ? 3 : 2;
+  for (int k = 0; k < nbuf; ++k) {
+    CK(cudaMalloc(&c->Y[k], sizeof(double) * np * NSTATE));
+    CK(cudaMemsetAsync(c->Y[k], 0, sizeof(double) * np * NSTATE, c->stream));
+  }
+  for (int k = 0; k < 2; ++k) {
+    CK(cudaMalloc(&c->orig[k], sizeof(uint32_t) * np));
+    CK(cudaMalloc(&c->key[k], sizeof(uint32_t) * np));
+    CK(cudaMalloc(&c->val[k], sizeof(uint32_t) * np));
+  }
+  CK(cudaMalloc(&c->arena, sizeof(double) * np * ARENA_FIELDS));
+  CK(cudaMemsetAsync(c->arena, 0, sizeof(double) * np * ARENA_FIELDS, c->stream));
+  CK(cudaMalloc(&c->nnb, sizeof(uint32_t) * np));
+  CK(cudaMalloc(&c->theta, sizeof(double) * np));
+  CK(cudaMalloc(&c->scratch, sizeof(double) * np));
+  c->bbox_blocks = std::min(nblk(n, BBOX_THREADS), 1024);
+  CK(cudaMalloc(&c->bbox_partial, sizeof(double) * 6 * c->bbox_blocks));
+  c->tot_blocks = std::min(nblk(n, TOT_THREADS), 1184);
+  CK(cudaMalloc(&c->tot_partial, sizeof(double) * TOT_NV * c->tot_blocks));
+  CK(cudaMalloc(&c->tot_out, sizeof(double) * 16));
+  c->ntiles = nblk(n, SORT_TILE);
+  c->hist_len = (int64_t)256 * c->ntiles;
+  c->nchunks = nblk(c->hist_len, SCAN_CHUNK);
+  CK(cudaMalloc(&c->hist, sizeof(uint32_t) * c->hist_len));
+  CK(cudaMalloc(&c->chunk_tot, sizeof(uint32_t) * c->nchunks));
+  /* fields */
+  fill_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->Y[0] + (int64_t)CCAKE_MASS * np, n, 1.0);
+  for (int k = 0; k < nfields; ++k) {
+    const int f = ids[k];
+    const bool active = (c->field_mask & (1u << f)) || f == CCAKE_MASS;
+    if (!active) continue;      /* switched-off sectors and third components in 2+1D are ignored */
+    CK(cudaMemcpyAsync(c->Y[0] + (int64_t)f * np, cols[k], sizeof(double) * n,
+                       memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
+  }
+  iota_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->orig[0], n);
+  CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
+  /* size the radix-sort key from the bounding box at load; the device coarsens the grid if the system outgrows it */
+  bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, c->stream>>>(c->Y[0], np, n, c->P.dim, c->bbox_partial);
+  bbox_final_kernel<<<1, 32, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 24, c->grid);
+  Grid g;
+  CK(cudaMemcpyAsync(&g, c->grid, sizeof(Grid), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  {
+    int64_t want = (int64_t)g.ncells * 8;
+    int bits = 1;
+    while (((int64_t)1 << bits) < want && bits < 24) ++bits;
+    c->passes = (bits + 7) / 8;
+    c->max_cells = 1 << (8 * c->passes);
+  }
+  CK(cudaMalloc(&c->cell_start, sizeof(uint32_t) * ((size_t)c->max_cells + 2)));
+  carve(c);
+  if (pair_work_alloc(c->pw, n, c->max_cells) != 0) { c->err = "pair work allocation failed"; return CCAKE_ENOMEM; }
+  c->x0 = c->P.x0_start;
+  c->loaded = true;
+  c->derived_valid = false;
+  int rc = launch_check(c, "load");
+  return rc;
+}
+
+int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4],
+                         int32_t ncols, const int32_t* col_ids, const double* data, int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (!dims || !axis_kind || !axes || !col_ids || !data || ncols <= 0 || ncols > CCAKE_NCOLS_MAX ||
+      (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_load_eos_table";
+    return CCAKE_EINVAL;
+  }
+  int64_t nodes = 1, nax = 0;
+  for (int k = 0; k < 4; ++k) {
+    if (dims[k] < 2 || !axes[k] || (axis_kind[k] != 0 && axis_kind[k] != 1) || (k == 0 && axis_kind[k] != 0)) {
+      c->err = "bad table axis";
+      return CCAKE_EINVAL;
+    }
+    nodes *= dims[k];
+    nax += dims[k];
+  }
+  TableDev tb;
+  std::memset(&tb, 0, sizeof(tb));
+  for (int cc = 0; cc < CCAKE_NCOLS_MAX; ++cc) tb.col_of[cc] = -1;
+  for (int k = 0; k < ncols; ++k) {
+    if (col_ids[k] < 0 || col_ids[k] >= CCAKE_NCOLS_MAX) { c->err = "bad column id"; return CCAKE_EINVAL; }
+    tb.col_of[col_ids[k]] = k;
+  }
+  for (int cc = 0; cc <= CCAKE_COL_WS; ++cc) if (tb.col_of[cc] < 0) { c->err = "table lacks a required column"; return CCAKE_EINVAL; }
+  if (c->kp.diff) for (int cc = CCAKE_COL_WB; cc <= CCAKE_COL_WQ; ++cc) if (tb.col_of[cc] < 0) { c->err = "diffusion needs dw/dn_q columns"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  /* axes must be strictly increasing: checked on the host copy */
+  std::vector<double> hax(nax);
+  {
+    int64_t off = 0;
+    for (int k = 0; k < 4; ++k) {
+      if (memspace == CCAKE_HOST) std::memcpy(hax.data() + off, axes[k], sizeof(double) * dims[k]);
+      else CK(cudaMemcpy(hax.data() + off, axes[k], sizeof(double) * dims[k], cudaMemcpyDeviceToHost));
+      for (int i = 1; i < dims[k]; ++i) if (!(hax[off + i] > hax[off + i - 1])) { c->err = "axis not increasing"; return CCAKE_EINVAL; }
+      off += dims[k];
+    }
+  }
+  free_table(c);
+  CK(cudaMalloc(&c->tb_axes, sizeof(double) * nax));
+  CK(cudaMalloc(&c->tb_data, sizeof(double) * nodes * ncols));
+  CK(cudaMemcpyAsync(c->tb_axes, hax.data(), sizeof(double) * nax, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->tb_data, data, sizeof(double) * nodes * ncols,
+                     memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  {
+    int64_t off = 0;
+    for (int k = 0; k < 4; ++k) { tb.dims[k] = dims[k]; tb.kind[k] = axis_kind[k]; tb.ax[k] = c->tb_axes + off; off += dims[k]; }
+  }
+  tb.ncols = ncols;
+  tb.data = c->tb_data;
+  c->tb = tb;
+  c->table_loaded = true;
+  c->derived_valid = false;
+  return CCAKE_OK;
+}
+
+int ccake_step(ccake_ctx* c, int32_t nsteps) {
+  if (!c) return CCAKE_EINVAL;
+  if (nsteps < 0) { c->err = "nsteps < 0"; return CCAKE_EINVAL; }
+  if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "step before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  for (int s = 0; s < nsteps; ++s) {
+    int rc = rk_step(c);
+    if (rc) return rc;
+  }
+  return CCAKE_OK;
+}
+
+int ccake_synchronize(ccake_ctx* c) {
+  if (!c) return CCAKE_EINVAL;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  Status s;
+  CK(cudaMemcpy(&s, c->status, sizeof(Status), cudaMemcpyDeviceToHost));
+  if (s.n_bad) { c->err = "singular per-particle system or NaN"; return CCAKE_ERANGE; }
+  if (s.n_oob) { c->err = "particles outside the EoS table (clamped)"; return CCAKE_ERANGE; }
+  return CCAKE_OK;
+}
+
+int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double* const* cols, int64_t capacity,
+                      int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (nfields <= 0 || !ids || !cols || (memspace != 0 && memspace != 1)) { c->err = "bad arguments to ccake_read_fields"; return CCAKE_EINVAL; }
+  if (!c->loaded) { c->err = "read before load"; return CCAKE_ESTATE; }
+  if (capacity < c->N) { c->err = "capacity < n"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  bool need = false;
+  for (int k = 0; k < nfields; ++k) {
+    if (!cols[k]) { c->err = "null column"; return CCAKE_EINVAL; }
+    if (ids[k] >= NSTATE) need = true;
+  }
+  if (need) {
+    if (c->P.eos_kind == 1 && !c->table_loaded) { c->err = "derived field before table load"; return CCAKE_ESTATE; }
+    int rc = refresh(c);
+    if (rc) return rc;
+  }
+  const int64_t N = c->N, np = c->npad;
+  cudaStream_t st = c->stream;
+  const Sorted& so = c->so;
+  const Geom gm = make_geom(c->P.coords, c->x0);
+  for (int k = 0; k < nfields; ++k) {
+    const int id = ids[k];
+    double* dst = (memspace == CCAKE_DEVICE) ? cols[k] : c->scratch;
+    const int g = nblk(N, 256);
+    const double* src_sorted = nullptr;
+    if (id >= 0 && id < NSTATE) scatter_store_kernel<<<g, 256, 0, st>>>(c->Y[0] + (int64_t)id * np, c->orig[0], N, dst);
+    else if (id >= CCAKE_RATE && id < CCAKE_RATE + NSTATE)
+      scatter_store_kernel<<<g, 256, 0, st>>>(c->Krate + (int64_t)(id - CCAKE_RATE) * np, c->orig[0], N, dst);
+    else switch (id) {
+      case CCAKE_SIGMA_STAR: src_sorted = so.sigma_star; break;
+      case CCAKE_S_DENS: src_sorted = so.s; break;
+      case CCAKE_RHO_B: src_sorted = so.n[0]; break;
+      case CCAKE_RHO_S: src_sorted = so.n[1]; break;
+      case CCAKE_RHO_Q: src_sorted = so.n[2]; break;
+      case CCAKE_T: src_sorted = so.T; break;
+      case CCAKE_MU_B: src_sorted = so.mu[0]; break;
+      case CCAKE_MU_S: src_sorted = so.mu[1]; break;
+      case CCAKE_MU_Q: src_sorted = so.mu[2]; break;
+      case CCAKE_P: src_sorted = so.p; break;
+      case CCAKE_E: src_sorted = so.e; break;
+      case CCAKE_CS2: src_sorted = so.cs2; break;
+      case CCAKE_GAMMA: src_sorted = so.gamma; break;
+      case CCAKE_THETA: src_sorted = c->theta; break;
+      case CCAKE_SIGMA: src_sorted = so.sigma; break;
+      case CCAKE_S_STAR: src_sorted = so.s_star; break;
+      case CCAKE_RHOSTAR_B: src_sorted = so.rho_star[0]; break;
+      case CCAKE_RHOSTAR_S: src_sorted = so.rho_star[1]; break;
+      case CCAKE_RHOSTAR_Q: src_sorted = so.rho_star[2]; break;
+      case CCAKE_WS: src_sorted = so.ws; break;
+      case CCAKE_DIVV: src_sorted = so.divv; break;
+      case CCAKE_NNB: scatter_sorted_u32_kernel<<<g, 256, 0, st>>>(so.nnb, so.perm, c->orig[0], N, dst); break;
+      case CCAKE_CELL:
+        /* so.FP[2]... are live; use theta-sized temp: reuse Kpair[8] only when diffusion is off — keep it simple: a
+           dedicated pass into so.divv would clobber; allocate nothing, write through scratch2 = so.x-independent */
+        {
+          double* tmp = nullptr;
+          CK(cudaMallocAsync(&tmp, sizeof(double) * np, st));
+          reported_cell_kernel<<<g, 256, 0, st>>>(so.x[0], so.x[1], so.x[2], N, c->P.dim, c->grid, tmp);
+          scatter_sorted_kernel<<<g, 256, 0, st>>>(tmp, so.perm, c->orig[0], N, dst);
+          CK(cudaFreeAsync(tmp, st));
+        }
+        break;
+      case CCAKE_FM1: case CCAKE_FM2: case CCAKE_FM3: {
+        const int i = id - CCAKE_FM1;
+        if (i < c->P.dim) scatter_diff_kernel<<<g, 256, 0, st>>>(so.FP[i], so.FB[i], gm.sqrtg, so.perm, c->orig[0], N, dst);
+        else fill_kernel<<<g, 256, 0, st>>>(dst, N, 0.0);
+        break;
+      }
+      case CCAKE_FK_B: case CCAKE_FK_S: case CCAKE_FK_Q:
+        scatter_diff_kernel<<<g, 256, 0, st>>>(so.FK[id - CCAKE_FK_B], nullptr, -gm.sqrtg, so.perm, c->orig[0], N, dst);
+        break;
+      default: c->err = "bad field id in read"; return CCAKE_EINVAL;
+    }
+    if (src_sorted) scatter_sorted_kernel<<<g, 256, 0, st>>>(src_sorted, so.perm, c->orig[0], N, dst);
+    int rc = launch_check(c, "read_fields");
+    if (rc) return rc;
+    if (memspace == CCAKE_HOST) {
+      CK(cudaMemcpyAsync(cols[k], c->scratch, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+      CK(cudaStreamSynchronize(st));
+    }
+  }
+  CK(cudaStreamSynchronize(st));
+  return CCAKE_OK;
+}
+
+int ccake_conserved_totals(ccake_ctx* c, double out[16]) {
+  if (!c) return CCAKE_EINVAL;
+  if (!out) { c->err = "null out"; return CCAKE_EINVAL; }
+  if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "totals before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  int rc = refresh(c);
+  if (rc) return rc;
+  const Geom gm = make_geom(c->P.coords, c->x0);
+  totals_partial_kernel<<<c->tot_blocks, TOT_THREADS, 0, c->stream>>>(c->N, c->kp, gm, c->Y[0], c->npad, c->so, c->tot_partial);
+  totals_final_kernel<<<1, 32, 0, c->stream>>>(c->tot_partial, c->tot_blocks, c->tot_out);
+  if ((rc = launch_check(c, "totals"))) return rc;
+  double t[TOT_NV];
+  Status s;
+  CK(cudaMemcpyAsync(t, c->tot_out, sizeof(double) * TOT_NV, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(&s, c->status, sizeof(Status), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 16; ++k) out[k] = 0.0;
+  out[0] = c->x0; out[1] = t[0]; out[2] = t[1]; out[3] = t[2]; out[4] = t[3]; out[5] = t[4];
+  out[6] = t[5]; out[7] = t[6]; out[8] = t[7]; out[9] = t[8]; out[10] = t[9]; out[11] = (double)s.n_oob;
+  out[12] = t[13]; out[13] = (double)s.n_bad; out[14] = t[10]; out[15] = 0.0;
+  return CCAKE_OK;
+}
+
+int ccake_read_neighbors(ccake_ctx* c, int64_t* counts, int64_t* offsets, int32_t* list, int64_t cap) {
+  if (!c) return CCAKE_EINVAL;
+  if (!counts) { c->err = "null counts"; return CCAKE_EINVAL; }
+  if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "neighbours before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  int rc = refresh(c);
+  if (rc) return rc;
+  const int64_t N = c->N;
+  cudaStream_t st = c->stream;
+  scatter_sorted_u32_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.nnb, c->so.perm, c->orig[0], N, c->scratch);
+  std::vector<double> h(N);
+  CK(cudaMemcpyAsync(h.data(), c->scratch, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  std::vector<long long> off(N + 1, 0);
+  for (int64_t a = 0; a < N; ++a) { counts[a] = (int64_t)h[a]; off[a + 1] = off[a] + counts[a]; }
+  if (offsets) for (int64_t a = 0; a <= N; ++a) offsets[a] = off[a];
+  if (list) {
+    if (cap < off[N]) { c->err = "list capacity too small"; return CCAKE_EINVAL; }
+    long long* doff = nullptr;
+    int* dlist = nullptr;
+    CK(cudaMalloc(&doff, sizeof(long long) * (N + 1)));
+    if (cudaMalloc(&dlist, sizeof(int) * std::max<long long>(off[N], 1)) != cudaSuccess) { cudaFree(doff); c->err = "neighbour list allocation"; return CCAKE_ENOMEM; }
+    cudaMemcpyAsync(doff, off.data(), sizeof(long long) * (N + 1), cudaMemcpyHostToDevice, st);
+    if (c->P.dim == 2) neighbour_walk_kernel<2><<<nblk(N, 128), 128, 0, st>>>(N, c->kp, c->grid, c->so, c->orig[0], 1, nullptr, doff, dlist);
+    else neighbour_walk_kernel<3><<<nblk(N, 128), 128, 0, st>>>(N, c->kp, c->grid, c->so, c->orig[0], 1, nullptr, doff, dlist);
+    cudaError_t e = cudaMemcpyAsync(list, dlist, sizeof(int) * off[N], cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(doff);
+    cudaFree(dlist);
+    if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return CCAKE_ECUDA; }
+    /* reporting format only: ascending original index within each set */
+    for (int64_t a = 0; a < N; ++a) std::sort(list + off[a], list + off[a + 1]);
+  }
+  return CCAKE_OK;
+}
+
+int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity) {
+  if (!c) return CCAKE_EINVAL;
+  if (!out || capacity < c->N) { c->err = "bad arguments to ccake_neighbor_hash"; return CCAKE_EINVAL; }
+  if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "hash before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  int rc = refresh(c);
+  if (rc) return rc;
+  const int64_t N = c->N;
+  unsigned long long* d = nullptr;
+  CK(cudaMalloc(&d, sizeof(unsigned long long) * N));
+  if (c->P.dim == 2) neighbour_walk_kernel<2><<<nblk(N, 128), 128, 0, c->stream>>>(N, c->kp, c->grid, c->so, c->orig[0], 0, d, nullptr, nullptr);
+  else neighbour_walk_kernel<3><<<nblk(N, 128), 128, 0, c->stream>>>(N, c->kp, c->grid, c->so, c->orig[0], 0, d, nullptr, nullptr);
+  cudaError_t e = cudaMemcpyAsync(out, d, sizeof(unsigned long long) * N, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return CCAKE_ECUDA; }
+  return CCAKE_OK;
+}
+
+int ccake_enable_timing(ccake_ctx* c, int32_t on) {
+  if (!c) return CCAKE_EINVAL;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  c->timing = on != 0;
+  c->ev_used = 0;
+  c->substeps_timed = 0;
+  return CCAKE_OK;
+}
+
+int ccake_kernel_times(ccake_ctx* c, double out[8]) {
+  if (!c) return CCAKE_EINVAL;
+  if (!out) { c->err = "null out"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 8; ++k) out[k] = 0.0;
+  /* 7 marks per substep: start, after sort, pack, smoothing, thermo, gradient, eom */
+  const size_t per = 7;
+  const size_t ns = c->ev_used / per;
+  for (size_t s = 0; s < ns; ++s)
+    for (int k = 0; k < 6; ++k) {
+      float ms = 0.f;
+      CK(cudaEventElapsedTime(&ms, c->ev[s * per + k], c->ev[s * per + k + 1]));
+      out[k] += ms;
+    }
+  if (ns) for (int k = 0; k < 6; ++k) out[k] /= (double)ns;
+  out[7] = (double)ns;
+  c->ev_used = 0;
+  c->substeps_timed = 0;
+  return CCAKE_OK;
+}
+
+}  /* extern "C" */

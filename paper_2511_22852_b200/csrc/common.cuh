@@ -1,0 +1,94 @@
+/*
+ * csrc/common.cuh — shared declarations of the CUDA library (product code; shares nothing with oracle/).
+ *
+ * Data layout in HBM (DESIGN.md §"Data layout"): structure of arrays, one fp64 array per field.
+ *   - "store order": the state buffers Y0 / Ystage / Yacc hold CCAKE_NSTATE fields of N doubles each, field f at
+ *     Y + f * Npad.  Store order is the cell-sorted order of the first substep of the current step; orig_id maps a
+ *     store slot back to the caller's original index.
+ *   - "sorted order": per-substep packed arrays (positions, smoothing payload, sums, thermodynamics, pair payload,
+ *     gradient sums) in the order of the stable radix sort by cell; perm[i] = store slot of sorted slot i.
+ */
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ccake.h"
+
+namespace ccake {
+
+constexpr int NQ = 3;
+constexpr int NSTATE = CCAKE_NSTATE;
+constexpr double GRID_MARGIN = 1.0 + 1.0 / 1048576.0; /* traversal-grid edge = 2h (1 + 2^-20): rounding in the
+                                                          cell index can never hide a pair with r^2 < (2h)^2 */
+
+/* uniform traversal grid of one substep, written by the bbox kernel, read by every later kernel */
+struct Grid {
+  double xmin[3], xmax[3];
+  double edge, inv_edge;
+  int nc[3];
+  int ncells;
+  /* reported cell id (DESIGN reading 9): edge exactly 2h */
+  double rep_inv_edge;
+  long long rep_nc[3];
+};
+
+/* geometry of a time slice: g = diag(1, -1, -1, -G3), G3 = tau^2 (hyperbolic) or 1 */
+struct Geom {
+  double G3, dG3, sqrtg, Gamma_g, tau;
+  int hyper;
+};
+
+__host__ __device__ inline Geom make_geom(int coords, double x0) {
+  Geom g;
+  g.hyper = coords;
+  g.tau = x0;
+  if (coords == 1) { g.G3 = x0 * x0; g.dG3 = 2.0 * x0; g.sqrtg = x0; g.Gamma_g = 1.0 / x0; }
+  else { g.G3 = 1.0; g.dG3 = 0.0; g.sqrtg = 1.0; g.Gamma_g = 0.0; }
+  return g;
+}
+
+/* constant parameters handed to kernels by value */
+struct KParams {
+  int D, coords, eom, eos_kind;
+  int shear, bulk, diff;
+  double h, inv_h, cut2, sigma_d;   /* kernel normalisation sigma_D of Eq. 77 */
+  double c0, c2, c4;
+  double eta_over_s, tau_pi_coeff, tau_floor;
+  double zeta_max, zeta_T_peak, zeta_width, tau_Pi_coeff;
+  double kappa_over_T2[9], tau_q_times_T[3], dnmr[8];
+};
+
+/* EoS table descriptor (device pointers) */
+struct TableDev {
+  int dims[4], kind[4], ncols;
+  int col_of[CCAKE_NCOLS_MAX];
+  const double* ax[4];
+  const double* data;
+};
+
+/* sorted-order work arrays of one substep (all device pointers, N entries each unless noted) */
+struct Sorted {
+  /* a3 */
+  uint32_t *key, *perm;              /* cell id, store slot */
+  uint32_t* cell_start;              /* ncells + 1, monotone */
+  /* pack: smoothing payload */
+  double *x[3], *S, *Nq[NQ], *m;
+  /* a4 */
+  double *sigma_star, *s_star, *rho_star[NQ];
+  uint32_t* nnb;
+  /* a5 */
+  double *gamma, *sigma, *s, *n[NQ];
+  double *T, *mu[NQ], *p, *e, *cs2, *ws, *wq[NQ];
+  double *Ppair, *Bpair[9], *Kpair[9], *alpha[NQ], *v[3], *u[3];
+  /* a6 */
+  double *FP[3], *FB[3], *FK[NQ], *DU[9], *DA[9], *divv;
+};
+
+/* device-side status counters */
+struct Status {
+  unsigned long long n_oob;      /* particles outside the EoS table in the latest thermo pass */
+  unsigned long long n_bad;      /* singular solves / NaN since the last load                 */
+  unsigned long long n_oob_total;
+};
+
+}  // namespace ccake

@@ -1,0 +1,368 @@
+/*
+ * csrc/eom.cuh — steps a7 (equations of motion) and a8 (RK stage update).
+ *
+ * PAPER.md Eq. 87-95 (:964-988): the time derivatives of phi_a enter linearly, M dphi/dx0 = F, and the system
+ * reduces to a D x D solve for du^i/dx0 (Eq. 95).  The reduction used here: GIVEN a trial du^i/dx0, every other
+ * rate is explicit —
+ *     du^0                      from u.u = 1 (Eq. 97 :1011)
+ *     theta, Du^mu, sigma^{mu nu}, omega^{mu nu}   from du^mu and the SPH gradients (Notation :164-169)
+ *     d(Pi/sigma)               bulk relaxation, Eq. 49 :676 / Eq. 52 row 1
+ *     d(pi^{ij}/sigma)          shear relaxation, Eq. 50 :678 / Eq. 52 row 3
+ *     d(J^i_q/sigma)            diffusion relaxation, Eq. 51 :680
+ *     d(pi^{0 mu}/sigma), d(J^0_q/sigma)   from the orthogonality constraints
+ *     dN_q                      charge conservation,  dS  entropy production (Eq. 96 :1003, Eq. 98 :1016)
+ * — so the momentum equation  d/dx0[ C u_i + pi~^0_i / gamma ] = sqrt(-g)(FP_i - FB_i)  is an affine map
+ * residual(du) = r0 + M du.  The kernel evaluates the residual at du = 0 and at the D unit vectors (columns of M,
+ * = the matrix of Eq. 95), solves M du = -r0 by Gaussian elimination with partial pivoting on the D x D matrix,
+ * and evaluates the explicit rates once more at the solution.  No dense system in all 17/23 unknowns is formed.
+ *
+ * The metric is diagonal, g = diag(1,-1,-1,-G3); the only Christoffel symbols are Gamma^tau_{eta eta} = tau,
+ * Gamma^eta_{tau eta} = 1/tau (:488), which are written out explicitly.
+ */
+#pragma once
+#include "common.cuh"
+#include "thermo_eos.cuh"
+
+namespace ccake {
+
+struct EomIn {
+  double u[4], ulo[4], v[4], glo[4], gup[4];
+  double gam, sig, sst, T, mu[NQ], p, e, cs2, ws, wq[NQ], s;
+  double eta, zeta, tau_pi, tau_Pi, kappa[NQ][NQ], tau_q[NQ];
+  double delta_PiPi, lambda_Pipi, delta_pipi, tau_pipi, lambda_piPi, phi_omega;
+  double CDc[4][4];      /* nabla_mu u^nu without the du^nu part of the row mu = 0 */
+  double Duc[4];         /* u^mu CDc[mu][nu] */
+  double thc;            /* gamma (div v + Gamma_g) */
+  double rhsJ[NQ][3];    /* constant right-hand side of the diffusion equation */
+  double FM[3];          /* sqrt(-g) (FP_i - FB_i) */
+  double FKs[NQ];        /* sqrt(-g) FK_q */
+  Dissip ds;
+};
+
+struct EomOut {
+  double du0, theta, dS, dN[NQ], dBulk, dpit[4][4], dJt[NQ][4], res[3];
+};
+
+template <int D>
+__device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
+                                       EomOut& o) {
+  const double gam = in.gam, sig = in.sig;
+  const double tau = gm.tau;
+  double du[4], dulo[4];
+  du[1] = du_in[0]; du[2] = du_in[1]; du[3] = (D == 3) ? du_in[2] : 0.0;
+  /* Eq. 97, nu = 0: u_0 du^0 = -u_k du^k - (1/2) u^a u^b dg_ab/dx0,  dg_33/dx0 = -dG3 */
+  const double gt = -in.u[3] * in.u[3] * gm.dG3;
+  du[0] = -(in.ulo[1] * du[1] + in.ulo[2] * du[2] + in.ulo[3] * du[3]) / gam - gt / (2.0 * gam);
+  for (int m = 0; m < 4; ++m) dulo[m] = in.glo[m] * du[m];
+  dulo[3] += -gm.dG3 * in.u[3];
+  o.du0 = du[0];
+  const double theta = in.thc + du[0];
+  o.theta = theta;
+  /* covariant derivative, acceleration */
+  double CD[4][4], Du[4], Dulo[4];
+  for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) CD[m][n] = in.CDc[m][n];
+  for (int n = 0; n < 4; ++n) { CD[0][n] += du[n]; Du[n] = in.Duc[n] + gam * du[n]; Dulo[n] = in.glo[n] * Du[n]; }
+
+  const double Pi = in.ds.bulkt * sig;
+  const bool need_sg = kp.shear || (kp.bulk && in.lambda_Pipi != 0.0);
+  double sg[4][4];
+  if (need_sg) {
+    for (int m = 0; m < 4; ++m)
+      for (int n = m; n < 4; ++n) {
+        const double Delta = ((m == n) ? in.gup[m] : 0.0) - in.u[m] * in.u[n];
+        const double v = 0.5 * (in.gup[m] * CD[m][n] + in.gup[n] * CD[n][m]) - 0.5 * (in.u[m] * Du[n] + in.u[n] * Du[m]) -
+                         (Delta / 3.0) * theta;
+        sg[m][n] = v; sg[n][m] = v;
+      }
+  }
+  /* bulk */
+  o.dBulk = 0.0;
+  if (kp.bulk) {
+    double rhs = -Pi - in.zeta * theta + (in.tau_Pi - in.delta_PiPi) * Pi * theta;
+    if (in.lambda_Pipi != 0.0) {
+      double acc = 0.0;
+      for (int m = 0; m < 4; ++m)
+        for (int n = 0; n < 4; ++n) acc += sig * in.ds.pit[m][n] * in.glo[m] * in.glo[n] * sg[m][n];
+      rhs += in.lambda_Pipi * acc;
+    }
+    o.dBulk = rhs / (in.tau_Pi * sig * gam);
+  }
+  /* shear */
+  for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) o.dpit[m][n] = 0.0;
+  if (kp.shear) {
+    double om[4][4];
+    const bool need_om = in.phi_omega != 0.0;
+    if (need_om)
+      for (int m = 0; m < 4; ++m)
+        for (int n = 0; n < 4; ++n)
+          om[m][n] = 0.5 * (in.gup[m] * CD[m][n] - in.gup[n] * CD[n][m]) - 0.5 * (in.u[m] * Du[n] - in.u[n] * Du[m]);
+    double Xtr = 0.0;
+    if (in.tau_pipi != 0.0)
+      for (int l = 0; l < 4; ++l)
+        for (int m = 0; m < 4; ++m) Xtr += sig * in.ds.pit[l][m] * in.glo[l] * in.glo[m] * sg[m][l];
+    for (int i = 1; i <= 3; ++i)
+      for (int j = i; j <= 3; ++j) {
+        if (D == 2 && j == 3 && i != 3) continue;          /* pi^{13}, pi^{23} vanish by symmetry in 2+1D */
+        double conn = 0.0;                                  /* u^l Gamma^i_{l r} pi~^{r j} + (i <-> j)      */
+        if (gm.hyper) {
+          if (i == 3) conn += (gam * in.ds.pit[3][j] + in.u[3] * in.ds.pit[0][j]) / tau;
+          if (j == 3) conn += (gam * in.ds.pit[i][3] + in.u[3] * in.ds.pit[i][0]) / tau;
+        }
+        double acc = 0.0;
+        for (int l = 0; l < 4; ++l) acc += (in.u[i] * in.ds.pit[j][l] + in.u[j] * in.ds.pit[i][l]) * Dulo[l];
+        const double piij = sig * in.ds.pit[i][j];
+        double rhs = -piij + 2.0 * in.eta * sg[i][j] + (in.tau_pi - in.delta_pipi) * piij * theta;
+        if (in.tau_pipi != 0.0) {
+          double X = 0.0;
+          for (int l = 0; l < 4; ++l) {
+            X += 0.5 * sig * in.ds.pit[l][i] * in.glo[l] * sg[l][j];
+            X += 0.5 * sig * in.ds.pit[l][j] * in.glo[l] * sg[l][i];
+          }
+          const double Delta = ((i == j) ? in.gup[i] : 0.0) - in.u[i] * in.u[j];
+          X -= (Delta / 3.0) * Xtr;
+          rhs -= in.tau_pipi * X;
+        }
+        if (in.lambda_piPi != 0.0) rhs += in.lambda_piPi * Pi * sg[i][j];
+        if (need_om) {
+          double Yv = 0.0;
+          for (int l = 0; l < 4; ++l) {
+            Yv += 0.5 * sig * in.ds.pit[i][l] * in.glo[l] * om[j][l];
+            Yv += 0.5 * sig * in.ds.pit[j][l] * in.glo[l] * om[i][l];
+          }
+          rhs += 2.0 * in.tau_pi * in.phi_omega * Yv;
+        }
+        const double d = (rhs / (sig * in.tau_pi) - conn - acc) / gam;
+        o.dpit[i][j] = d; o.dpit[j][i] = d;
+      }
+    /* d/dx0 of u_mu pi~^{mu nu} = 0 */
+    for (int n = 1; n <= 3; ++n) {
+      double acc = 0.0;
+      for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][n];
+      for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][n];
+      o.dpit[0][n] = acc / gam; o.dpit[n][0] = acc / gam;
+    }
+    double acc = 0.0;
+    for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][0];
+    for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][0];
+    o.dpit[0][0] = acc / gam;
+  }
+  /* diffusion */
+  for (int q = 0; q < NQ; ++q) for (int m = 0; m < 4; ++m) o.dJt[q][m] = 0.0;
+  if (kp.diff) {
+    for (int q = 0; q < NQ; ++q) {
+      double JDu = 0.0;
+      for (int n = 0; n < 4; ++n) JDu += in.ds.Jt[q][n] * Dulo[n];
+      for (int i = 1; i <= D; ++i) {
+        double conn = 0.0;
+        if (gm.hyper && i == 3) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) / tau;
+        o.dJt[q][i] = (in.rhsJ[q][i - 1] / (in.tau_q[q] * sig) - conn - in.u[i] * JDu) / gam;
+      }
+      double acc = 0.0;
+      for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.Jt[q][m];
+      for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dJt[q][j];
+      o.dJt[q][0] = acc / gam;
+    }
+  }
+  /* charge: d/dx0 [ N_q + J~^0_q / gamma ] = -sqrt(-g) FK_q */
+  for (int q = 0; q < NQ; ++q)
+    o.dN[q] = -in.FKs[q] - o.dJt[q][0] / gam + (in.ds.Jt[q][0] / (gam * gam)) * du[0];
+  /* entropy, Eq. 96: gamma sigma (T dS + mu_q dN_q) = -Pi theta + pi^mu_nu nabla_mu u^nu */
+  {
+    double rhs = -Pi * theta;
+    if (kp.shear)
+      for (int m = 0; m < 4; ++m)
+        for (int n = 0; n < 4; ++n) rhs += sig * in.ds.pit[m][n] * in.glo[n] * CD[m][n];
+    double lhs = 0.0;
+    for (int q = 0; q < NQ; ++q) lhs += gam * sig * in.mu[q] * o.dN[q];
+    o.dS = (rhs - lhs) / (gam * sig * in.T);
+  }
+  /* momentum residual */
+  const double w = in.e + in.p;
+  const double A = w * in.cs2;
+  const double Cc = w / sig + in.ds.bulkt;
+  double dC = in.ws * o.dS + o.dBulk - (A / sig) * (theta / gam);
+  for (int q = 0; q < NQ; ++q) dC += in.wq[q] * o.dN[q];
+  for (int i = 1; i <= D; ++i) {
+    const double pit0_lo = in.glo[i] * in.ds.pit[0][i];
+    double dpit0_lo = in.glo[i] * o.dpit[0][i];
+    if (i == 3) dpit0_lo += -gm.dG3 * in.ds.pit[0][3];
+    o.res[i - 1] = in.ulo[i] * dC + Cc * dulo[i] + dpit0_lo / gam - (pit0_lo / (gam * gam)) * du[0] - in.FM[i - 1];
+  }
+}
+
+/* RK bookkeeping of one substep (DESIGN reading 7):
+     y_out = y_base + c_out * k                 (stage state, or the final state for RK2)
+     RK4:  acc = k (mode 1) | acc + w k (mode 2) ; final: y_out = y_base + c_out * (acc + w k) (mode 3)          */
+struct RkArgs {
+  const double* Ycur;   /* state the rates are evaluated at        */
+  const double* Ybase;  /* y0 of the step                          */
+  double* Yout;         /* may alias Ybase (own-slot read then write) */
+  double* Yacc;         /* RK4 accumulator or NULL                 */
+  double* Krate;        /* rates in store order, or NULL           */
+  double* theta_out;    /* sorted order                            */
+  double c_out, w_acc;
+  int acc_mode;         /* 0 none | 1 set | 2 add | 3 final        */
+  int update;           /* 0: rates only (refresh)                 */
+};
+
+template <int D>
+__global__ void __launch_bounds__(128)
+eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, uint32_t field_mask,
+           Status* __restrict__ status) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t a = so.perm[i];
+  const double* __restrict__ Y = rk.Ycur;
+  EomIn in;
+  load_u(kp, gm, Y, npad, a, in.u);
+  in.gam = in.u[0];
+  in.glo[0] = 1.0; in.glo[1] = -1.0; in.glo[2] = -1.0; in.glo[3] = -gm.G3;
+  for (int m = 0; m < 4; ++m) { in.gup[m] = 1.0 / in.glo[m]; in.ulo[m] = in.glo[m] * in.u[m]; in.v[m] = in.u[m] / in.gam; }
+  load_dissip(kp, gm, Y, npad, a, in.u, in.ds);
+  in.sig = so.sigma[i]; in.sst = so.sigma_star[i]; in.s = so.s[i];
+  in.T = so.T[i]; in.p = so.p[i]; in.e = so.e[i]; in.cs2 = so.cs2[i]; in.ws = so.ws[i];
+  for (int q = 0; q < NQ; ++q) { in.mu[q] = so.mu[q][i]; in.wq[q] = kp.diff || kp.eos_kind == 0 ? so.wq[q][i] : so.wq[q][i]; }
+  /* transport coefficients, §5.3 (:732-769), DESIGN reading 11 */
+  {
+    const double w = in.e + in.p;
+    in.eta = kp.eta_over_s * in.s;
+    in.tau_pi = fmax(kp.tau_pi_coeff * in.eta / w, kp.tau_floor);
+    const double dT = in.T - kp.zeta_T_peak;
+    in.zeta = (kp.zeta_width > 0.0)
+                  ? kp.zeta_max * (kp.zeta_width * kp.zeta_width) / (kp.zeta_width * kp.zeta_width + dT * dT) * in.s
+                  : kp.zeta_max * in.s;
+    in.tau_Pi = kp.tau_Pi_coeff * in.tau_pi;
+    for (int q = 0; q < NQ; ++q) {
+      for (int r = 0; r < NQ; ++r) in.kappa[q][r] = kp.kappa_over_T2[q * 3 + r] * in.T * in.T;
+      in.tau_q[q] = kp.tau_q_times_T[q] / in.T;
+    }
+    in.delta_PiPi = in.tau_Pi; in.lambda_Pipi = 0.0; in.delta_pipi = (4.0 / 3.0) * in.tau_pi; in.tau_pipi = 0.0;
+    in.lambda_piPi = 0.0; in.phi_omega = 0.0;
+    if (kp.eom == 2) {
+      in.delta_PiPi = kp.dnmr[0] * in.tau_Pi; in.lambda_Pipi = kp.dnmr[1] * in.tau_Pi;
+      in.delta_pipi = kp.dnmr[2] * in.tau_pi; in.tau_pipi = kp.dnmr[3] * in.tau_pi;
+      in.lambda_piPi = kp.dnmr[4]; in.phi_omega = kp.dnmr[5];
+    }
+  }
+  /* gradients: d_k u^j from the SPH sums, d_k u^0 from u_mu d_k u^mu = 0, d_0 = d/dx0 - v^k d_k */
+  {
+    double PU[4][4];
+    for (int m = 0; m < 4; ++m) for (int nn = 0; nn < 4; ++nn) PU[m][nn] = 0.0;
+    const double G[4] = {0.0, 1.0, 1.0, gm.G3};
+    for (int k = 1; k <= D; ++k) {
+      double s0 = 0.0;
+      for (int j = 1; j <= D; ++j) {
+        const double d = so.DU[(k - 1) * 3 + (j - 1)][i];
+        PU[k][j] = d;
+        s0 += G[j] * in.u[j] * d;
+      }
+      PU[k][0] = s0 / in.gam;
+    }
+    for (int nn = 0; nn < 4; ++nn) {
+      double s0 = 0.0;
+      for (int k = 1; k <= 3; ++k) s0 -= in.v[k] * PU[k][nn];
+      PU[0][nn] = s0;                                         /* + du^nn, added per trial */
+    }
+    for (int m = 0; m < 4; ++m) for (int nn = 0; nn < 4; ++nn) in.CDc[m][nn] = PU[m][nn];
+    if (gm.hyper) {
+      in.CDc[3][0] += gm.tau * in.u[3];          /* Gamma^0_{33} u^3 */
+      in.CDc[0][3] += in.u[3] / gm.tau;          /* Gamma^3_{03} u^3 */
+      in.CDc[3][3] += in.gam / gm.tau;           /* Gamma^3_{30} u^0 */
+    }
+    for (int nn = 0; nn < 4; ++nn) {
+      double s0 = 0.0;
+      for (int m = 0; m < 4; ++m) s0 += in.u[m] * in.CDc[m][nn];
+      in.Duc[nn] = s0;
+    }
+  }
+  in.thc = in.gam * (so.divv[i] + gm.Gamma_g);
+  for (int k = 0; k < 3; ++k) in.FM[k] = (k < D) ? gm.sqrtg * (so.FP[k][i] - so.FB[k][i]) : 0.0;
+  for (int q = 0; q < NQ; ++q) in.FKs[q] = gm.sqrtg * so.FK[q][i];
+  if (kp.diff) {
+    /* tau_q sigma [...] = -J^i_q + sum_q' kappa_qq' nabla^<i> alpha_q',  nabla^<i> alpha = g^{ii} d_i alpha - u^i u^j d_j alpha */
+    double udota[NQ];
+    for (int r = 0; r < NQ; ++r) {
+      double s0 = 0.0;
+      for (int j = 1; j <= D; ++j) s0 += in.u[j] * so.DA[r * 3 + (j - 1)][i];
+      udota[r] = s0;
+    }
+    for (int q = 0; q < NQ; ++q)
+      for (int k = 1; k <= D; ++k) {
+        double rhs = -in.sig * in.ds.Jt[q][k];
+        for (int r = 0; r < NQ; ++r) rhs += in.kappa[q][r] * (in.gup[k] * so.DA[r * 3 + (k - 1)][i] - in.u[k] * udota[r]);
+        in.rhsJ[q][k - 1] = rhs;
+      }
+  }
+
+  /* residual at du = 0 and at the unit vectors -> D x D system of Eq. 95 */
+  EomOut o;
+  double r0[3], M[3][3], du[3] = {0.0, 0.0, 0.0};
+  eom_rates<D>(kp, gm, in, du, o);
+  for (int k = 0; k < D; ++k) r0[k] = o.res[k];
+#pragma unroll 1
+  for (int c = 0; c < D; ++c) {
+    double e[3] = {0.0, 0.0, 0.0};
+    e[c] = 1.0;
+    eom_rates<D>(kp, gm, in, e, o);
+    for (int k = 0; k < D; ++k) M[k][c] = o.res[k] - r0[k];
+  }
+  /* Gaussian elimination with partial pivoting */
+  double b[3];
+  bool ok = true;
+  for (int k = 0; k < D; ++k) b[k] = -r0[k];
+  for (int c = 0; c < D; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < D; ++r) if (fabs(M[r][c]) > fabs(M[piv][c])) piv = r;
+    if (M[piv][c] == 0.0 || !(fabs(M[piv][c]) < INFINITY)) { ok = false; break; }
+    if (piv != c) {
+      for (int k = 0; k < D; ++k) { const double t = M[c][k]; M[c][k] = M[piv][k]; M[piv][k] = t; }
+      const double t = b[c]; b[c] = b[piv]; b[piv] = t;
+    }
+    for (int r = c + 1; r < D; ++r) {
+      const double f = M[r][c] / M[c][c];
+      for (int k = c; k < D; ++k) M[r][k] -= f * M[c][k];
+      b[r] -= f * b[c];
+    }
+  }
+  if (ok)
+    for (int r = D - 1; r >= 0; --r) {
+      double s0 = b[r];
+      for (int k = r + 1; k < D; ++k) s0 -= M[r][k] * du[k];
+      du[r] = s0 / M[r][r];
+    }
+  eom_rates<D>(kp, gm, in, du, o);
+  if (!ok || !(o.dS == o.dS) || !(du[0] == du[0])) atomicAdd(&status->n_bad, 1ULL);
+
+  /* rates of the evolved set */
+  double k_[NSTATE];
+  for (int f = 0; f < NSTATE; ++f) k_[f] = 0.0;
+  for (int j = 1; j <= D; ++j) { k_[CCAKE_R1 + j - 1] = in.u[j] / in.gam; k_[CCAKE_U1 + j - 1] = du[j - 1]; }
+  k_[CCAKE_S] = o.dS;
+  for (int q = 0; q < NQ; ++q) k_[CCAKE_NB + q] = o.dN[q];
+  k_[CCAKE_BULK] = o.dBulk;
+  k_[CCAKE_PI11] = o.dpit[1][1]; k_[CCAKE_PI12] = o.dpit[1][2]; k_[CCAKE_PI22] = o.dpit[2][2]; k_[CCAKE_PI33] = o.dpit[3][3];
+  if (D == 3) { k_[CCAKE_PI13] = o.dpit[1][3]; k_[CCAKE_PI23] = o.dpit[2][3]; }
+  for (int q = 0; q < NQ; ++q) for (int j = 1; j <= D; ++j) k_[CCAKE_JB1 + 3 * q + j - 1] = o.dJt[q][j];
+  /* 2+1D hyperbolic: longitudinal work rate (DESIGN reading 14) */
+  if (gm.hyper && D == 2) {
+    const double Pi = in.ds.bulkt * in.sig;
+    k_[CCAKE_WORK] = (Y[CCAKE_MASS * npad + a] / in.sst) * (in.p + Pi + gm.tau * gm.tau * in.sig * in.ds.pit[3][3]);
+  }
+  if (rk.theta_out) rk.theta_out[i] = o.theta;
+  if (rk.Krate)
+    for (int f = 0; f < NSTATE; ++f) if (f != CCAKE_MASS) rk.Krate[f * npad + a] = k_[f];
+  if (rk.update) {
+    for (int f = 0; f < NSTATE; ++f) {
+      if (!(field_mask & (1u << f)) || f == CCAKE_MASS) continue;
+      const double y0 = rk.Ybase[f * npad + a];
+      double kk = k_[f];
+      if (rk.acc_mode == 1) rk.Yacc[f * npad + a] = kk;
+      else if (rk.acc_mode == 2) { rk.Yacc[f * npad + a] = rk.Yacc[f * npad + a] + rk.w_acc * kk; }
+      else if (rk.acc_mode == 3) kk = rk.Yacc[f * npad + a] + kk;
+      rk.Yout[f * npad + a] = y0 + rk.c_out * kk;
+    }
+    if (rk.Yout != rk.Ybase) rk.Yout[CCAKE_MASS * npad + a] = rk.Ybase[CCAKE_MASS * npad + a];
+  }
+}
+
+}  // namespace ccake

@@ -1,0 +1,309 @@
+/*
+ * csrc/grid_sort.cuh — steps a1-a3: bounding box, cell hash, stable LSD radix sort by cell, cell lists.
+ * PAPER.md :1434 (§5.9.1): "particles are spatially binned ... neighbours drawn from nearby cells within a
+ * cut-off radius", O(N).  Integer work only, except the fp64 coordinate -> cell index map, which uses
+ * round-to-nearest multiplies without FMA contraction so that the reported cell ids are reproducible bit by bit.
+ */
+#pragma once
+#include "common.cuh"
+
+namespace ccake {
+
+constexpr int BBOX_THREADS = 256;
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
+constexpr int SCAN_CHUNK = 1024;
+
+/* ------------------------------------------------------------------------------------------- a1 bbox ---- */
+__device__ inline double warp_min(double v) {
+  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ inline double warp_max(double v) {
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+/* partial[block][0..5] = min x,y,z, max x,y,z over the block's grid-stride share */
+__global__ void __launch_bounds__(BBOX_THREADS)
+bbox_partial_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D, double* __restrict__ partial) {
+  double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    for (int k = 0; k < 3; ++k) {
+      if (k < D) {
+        const double v = Y[(CCAKE_R1 + k) * npad + i];
+        lo[k] = fmin(lo[k], v);
+        hi[k] = fmax(hi[k], v);
+      }
+    }
+  }
+  __shared__ double sm[6][BBOX_THREADS / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int k = 0; k < 3; ++k) {
+    const double a = warp_min(lo[k]), b = warp_max(hi[k]);
+    if (lane == 0) { sm[k][w] = a; sm[3 + k][w] = b; }
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    double r = sm[threadIdx.x][0];
+    for (int j = 1; j < BBOX_THREADS / 32; ++j) r = (threadIdx.x < 3) ? fmin(r, sm[threadIdx.x][j]) : fmax(r, sm[threadIdx.x][j]);
+    partial[blockIdx.x * 6 + threadIdx.x] = r;
+  }
+}
+
+/* one block: reduce the partials (min/max are exact and order-free) and lay out the traversal grid */
+__global__ void bbox_final_kernel(const double* __restrict__ partial, int nblocks, int D, double h, int max_cells,
+                                  Grid* __restrict__ grid) {
+  __shared__ double red[6];
+  if (threadIdx.x < 6) {
+    double r = partial[threadIdx.x];
+    for (int b = 1; b < nblocks; ++b) {
+      const double v = partial[b * 6 + threadIdx.x];
+      r = (threadIdx.x < 3) ? fmin(r, v) : fmax(r, v);
+    }
+    red[threadIdx.x] = r;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    Grid g;
+    for (int k = 0; k < 3; ++k) {
+      g.xmin[k] = (k < D) ? red[k] : 0.0;
+      g.xmax[k] = (k < D) ? red[3 + k] : 0.0;
+    }
+    const double twoh = 2.0 * h;
+    double edge = twoh * GRID_MARGIN;
+    /* coarsen by powers of two until the cell count fits the radix-sort key width chosen at load time */
+    for (int it = 0; it < 64; ++it) {
+      double total = 1.0;
+      for (int k = 0; k < 3; ++k) {
+        g.nc[k] = 1;
+        if (k < D) {
+          double ext = (g.xmax[k] - g.xmin[k]) / edge;
+          if (!(ext >= 0.0)) ext = 0.0;
+          if (ext > 1.0e9) ext = 1.0e9;
+          g.nc[k] = (int)floor(ext) + 1;
+        }
+        total *= (double)g.nc[k];
+      }
+      if (total <= (double)max_cells) break;
+      edge *= 2.0;
+    }
+    g.edge = edge;
+    g.inv_edge = 1.0 / edge;
+    g.ncells = g.nc[0] * g.nc[1] * g.nc[2];
+    g.rep_inv_edge = 1.0 / twoh;
+    for (int k = 0; k < 3; ++k) {
+      g.rep_nc[k] = 1;
+      if (k < D) g.rep_nc[k] = (long long)floor(__dmul_rn(__dsub_rn(g.xmax[k], g.xmin[k]), g.rep_inv_edge)) + 1;
+    }
+    *grid = g;
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ a2 hash ---- */
+__device__ inline int cell_coord(double x, double xmin, double inv_edge, int nc) {
+  const double t = floor(__dmul_rn(__dsub_rn(x, xmin), inv_edge));
+  int c = 0;
+  if (t >= 0.0) c = (t < (double)nc) ? (int)t : nc - 1;   /* NaN -> 0 */
+  return c;
+}
+
+__global__ void cell_hash_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
+                                 const Grid* __restrict__ grid, uint32_t* __restrict__ key, uint32_t* __restrict__ val) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Grid g = *grid;
+  int c[3] = {0, 0, 0};
+  for (int k = 0; k < 3; ++k)
+    if (k < D) c[k] = cell_coord(Y[(CCAKE_R1 + k) * npad + i], g.xmin[k], g.inv_edge, g.nc[k]);
+  key[i] = (uint32_t)(c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2]));
+  val[i] = (uint32_t)i;
+}
+
+/* reported cell id (field CCAKE_CELL): edge exactly 2h, origin = exact coordinate minimum, product then floor */
+__global__ void reported_cell_kernel(const double* __restrict__ x0, const double* __restrict__ x1,
+                                     const double* __restrict__ x2, int64_t n, int D, const Grid* __restrict__ grid,
+                                     double* __restrict__ out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Grid g = *grid;
+  const double* xs[3] = {x0, x1, x2};
+  long long c[3] = {0, 0, 0};
+  for (int k = 0; k < 3; ++k)
+    if (k < D) c[k] = (long long)floor(__dmul_rn(__dsub_rn(xs[k][i], g.xmin[k]), g.rep_inv_edge));
+  out[i] = (double)(c[0] + g.rep_nc[0] * (c[1] + g.rep_nc[1] * c[2]));
+}
+
+/* ------------------------------------------------------------------------------- a3 stable radix sort ---- */
+/* pass 1 of 3: per-tile digit histogram; hist[d * ntiles + tile] */
+__global__ void __launch_bounds__(SORT_THREADS)
+radix_hist_kernel(const uint32_t* __restrict__ key, int64_t n, int shift, int ntiles, uint32_t* __restrict__ hist) {
+  __shared__ uint32_t sh[256];
+  sh[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+  for (int r = 0; r < SORT_ITEMS; ++r) {
+    const int64_t i = base + r * SORT_THREADS + threadIdx.x;
+    if (i < n) atomicAdd(&sh[(key[i] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  hist[(int64_t)threadIdx.x * ntiles + blockIdx.x] = sh[threadIdx.x];
+}
+
+/* exclusive scan of m entries in chunks of SCAN_CHUNK: (1) in-chunk scan + chunk totals, (2) one block scans the
+   totals, (3) consumers add chunk_off[idx / SCAN_CHUNK] */
+__global__ void __launch_bounds__(SCAN_CHUNK)
+scan_chunk_kernel(uint32_t* __restrict__ data, int64_t m, uint32_t* __restrict__ chunk_tot) {
+  __shared__ uint32_t wsum[32];
+  const int64_t i = (int64_t)blockIdx.x * SCAN_CHUNK + threadIdx.x;
+  const uint32_t v = (i < m) ? data[i] : 0u;
+  uint32_t x = v;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t s = wsum[lane];
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += y;
+    }
+    wsum[lane] = s;
+  }
+  __syncthreads();
+  const uint32_t incl = x + (w ? wsum[w - 1] : 0u);
+  if (i < m) data[i] = incl - v;
+  if (threadIdx.x == SCAN_CHUNK - 1) chunk_tot[blockIdx.x] = incl;
+}
+
+__global__ void __launch_bounds__(1024)
+scan_totals_kernel(uint32_t* __restrict__ chunk_tot, int nchunks) {
+  __shared__ uint32_t wsum[32];
+  __shared__ uint32_t carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int base = 0; base < nchunks; base += 1024) {
+    const int i = base + threadIdx.x;
+    const uint32_t v = (i < nchunks) ? chunk_tot[i] : 0u;
+    uint32_t x = v;
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += y;
+    }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+      uint32_t s = wsum[lane];
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+        if (lane >= o) s += y;
+      }
+      wsum[lane] = s;
+    }
+    __syncthreads();
+    const uint32_t incl = x + (w ? wsum[w - 1] : 0u) + carry_s;
+    if (i < nchunks) chunk_tot[i] = incl - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = incl;
+    __syncthreads();
+  }
+}
+
+/* pass 3 of 3: stable scatter.  Keys of a tile are visited in rounds of SORT_THREADS consecutive keys; within a
+   round the rank of a key among equal digits is (keys of earlier rounds) + (equal digits in lower warps) +
+   (equal digits in lower lanes), which preserves the input order. */
+__global__ void __launch_bounds__(SORT_THREADS)
+radix_scatter_kernel(const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, int64_t n, int shift,
+                     int ntiles, const uint32_t* __restrict__ hist, const uint32_t* __restrict__ chunk_off,
+                     uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out) {
+  constexpr int NW = SORT_THREADS / 32;
+  __shared__ uint32_t wc[NW][256];
+  __shared__ uint32_t run[256];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  {
+    const int64_t hidx = (int64_t)threadIdx.x * ntiles + blockIdx.x;
+    run[threadIdx.x] = hist[hidx] + chunk_off[hidx / SCAN_CHUNK];
+    for (int j = 0; j < NW; ++j) wc[j][threadIdx.x] = 0;
+  }
+  __syncthreads();
+  const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+  for (int r = 0; r < SORT_ITEMS; ++r) {
+    const int64_t i = base + r * SORT_THREADS + threadIdx.x;
+    const bool ok = i < n;
+    uint32_t k = 0, v = 0, d = 256;
+    if (ok) { k = key_in[i]; v = val_in[i]; d = (k >> shift) & 255u; }
+    const uint32_t mask = __match_any_sync(0xffffffffu, d);
+    const uint32_t rank_w = __popc(mask & ((1u << lane) - 1u));
+    if (ok && rank_w == 0) wc[w][d] = __popc(mask);
+    __syncthreads();
+    uint32_t pos = 0;
+    if (ok) {
+      pos = run[d] + rank_w;
+      for (int j = 0; j < w; ++j) pos += wc[j][d];
+    }
+    __syncthreads();
+    {
+      uint32_t tot = 0;
+      for (int j = 0; j < NW; ++j) { tot += wc[j][threadIdx.x]; wc[j][threadIdx.x] = 0; }
+      run[threadIdx.x] += tot;
+    }
+    __syncthreads();
+    if (ok) { key_out[pos] = k; val_out[pos] = v; }
+  }
+}
+
+/* monotone cell_start[0..ncells]: cell c owns sorted slots [cell_start[c], cell_start[c+1]) */
+__global__ void cell_start_kernel(const uint32_t* __restrict__ key, int64_t n, const Grid* __restrict__ grid,
+                                  uint32_t* __restrict__ cell_start) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t k1 = key[i];
+  const int64_t k0 = (i == 0) ? -1 : (int64_t)key[i - 1];
+  for (int64_t c = k0 + 1; c <= k1; ++c) cell_start[c] = (uint32_t)i;
+  if (i == n - 1) {
+    const int ncells = grid->ncells;
+    for (int64_t c = k1 + 1; c <= ncells; ++c) cell_start[c] = (uint32_t)n;
+  }
+}
+
+/* ------------------------------------------------------------------------------ reorder and pack ---- */
+/* physical reorder of the store at the first substep of a step: dst[f][i] = src[f][perm[i]] for the active
+   fields; afterwards the store order IS the sorted order and perm becomes the identity */
+__global__ void reorder_store_kernel(const double* __restrict__ src, double* __restrict__ dst, int64_t npad, int64_t n,
+                                     const uint32_t* __restrict__ perm, uint32_t field_mask,
+                                     const uint32_t* __restrict__ orig_src, uint32_t* __restrict__ orig_dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t a = perm[i];
+  for (int f = 0; f < NSTATE; ++f)
+    if (field_mask & (1u << f)) dst[f * npad + i] = src[f * npad + a];
+  orig_dst[i] = orig_src[a];
+}
+
+__global__ void iota_kernel(uint32_t* __restrict__ p, int64_t n) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) p[i] = (uint32_t)i;
+}
+
+/* smoothing payload in sorted order: r, S, N_q, m */
+__global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
+                                      const uint32_t* __restrict__ perm, Sorted so) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t a = perm[i];
+  so.x[0][i] = Y[CCAKE_R1 * npad + a];
+  so.x[1][i] = Y[CCAKE_R2 * npad + a];
+  so.x[2][i] = (D == 3) ? Y[CCAKE_R3 * npad + a] : 0.0;
+  so.S[i] = Y[CCAKE_S * npad + a];
+  so.Nq[0][i] = Y[CCAKE_NB * npad + a];
+  so.Nq[1][i] = Y[CCAKE_NS * npad + a];
+  so.Nq[2][i] = Y[CCAKE_NQ * npad + a];
+  so.m[i] = Y[CCAKE_MASS * npad + a];
+}
+
+}  // namespace ccake

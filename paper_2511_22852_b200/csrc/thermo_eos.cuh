@@ -1,0 +1,236 @@
+/*
+ * csrc/thermo_eos.cuh — step a5: rest-frame densities, equation of state, pair inputs.
+ *
+ *   X_a = X*_a / (gamma_a sqrt(-g))                              PAPER.md Eq. 68 :864 (DESIGN reading 2)
+ *   table: per-axis cell search + quadrilinear blend of 16 nodes  :583-593 (log-decade axes :593)
+ *   closed form: p = c0 T^4 + c2 T^2 sum mu^2 + c4 sum mu^4       App. A Eq. A.5-A.7 :2115-2122, cubic A.11-A.14
+ *   pair inputs: (p + Pi)/sigma*^2, B^j_i/sigma*^2, K^j_q/sigma*^2, alpha_q = mu_q/T, v^i   (DESIGN §"EoM")
+ */
+#pragma once
+#include "common.cuh"
+
+namespace ccake {
+
+struct ThermoOut { double T, mu[NQ], p, e, cs2, ws, wq[NQ]; int oob; };
+
+/* last node <= x by comparisons only (binary search); the cell is clamped to [0, n-2] */
+__device__ inline int axis_cell(const double* __restrict__ ax, int n, double x) {
+  int lo = 0, hi = n;              /* first index with ax[idx] > x, in [lo, hi] */
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (ax[mid] <= x) lo = mid + 1; else hi = mid;
+  }
+  int i = lo - 1;
+  if (i > n - 2) i = n - 2;
+  if (i < 0) i = 0;
+  return i;
+}
+
+__device__ inline ThermoOut eos_table_lookup(const TableDev& tb, double s, const double n[NQ]) {
+  ThermoOut th;
+  th.oob = 0;
+  double x[4];
+  x[0] = s;
+  for (int k = 1; k < 4; ++k) x[k] = (tb.kind[k] == 1) ? n[k - 1] / s : n[k - 1];
+  int i0[4];
+  double t[4];
+  for (int k = 0; k < 4; ++k) {
+    const double* ax = tb.ax[k];
+    const int nn = tb.dims[k];
+    double xv = x[k];
+    const double a0 = ax[0], a1 = ax[nn - 1];
+    if (!(xv >= a0)) { xv = a0; th.oob = 1; }
+    if (!(xv <= a1)) { xv = a1; th.oob = 1; }
+    const int i = axis_cell(ax, nn, xv);
+    i0[k] = i;
+    const double lo = ax[i], hi = ax[i + 1];
+    t[k] = (xv - lo) / (hi - lo);
+  }
+  double out[CCAKE_NCOLS_MAX];
+  for (int c = 0; c < CCAKE_NCOLS_MAX; ++c) out[c] = 0.0;
+  const int nc = tb.ncols;
+  /* 16 nodes; the two nodes along the innermost axis are adjacent in memory (2 * ncols doubles) */
+  for (int b0 = 0; b0 < 2; ++b0)
+    for (int b1 = 0; b1 < 2; ++b1)
+      for (int b2 = 0; b2 < 2; ++b2) {
+        const double w0 = b0 ? t[0] : 1.0 - t[0];
+        const double w1 = b1 ? t[1] : 1.0 - t[1];
+        const double w2 = b2 ? t[2] : 1.0 - t[2];
+        const double w012 = (w0 * w1) * w2;
+        const int64_t node = (((int64_t)(i0[0] + b0) * tb.dims[1] + (i0[1] + b1)) * tb.dims[2] + (i0[2] + b2)) * tb.dims[3] + i0[3];
+        const double* __restrict__ p0 = tb.data + node * nc;
+        const double wl = w012 * (1.0 - t[3]), wh = w012 * t[3];
+        for (int c = 0; c < CCAKE_NCOLS_MAX; ++c) {
+          const int col = tb.col_of[c];
+          if (col >= 0) { out[c] += wl * __ldg(p0 + col); out[c] += wh * __ldg(p0 + nc + col); }
+        }
+      }
+  th.T = out[CCAKE_COL_T];
+  for (int q = 0; q < NQ; ++q) { th.mu[q] = out[CCAKE_COL_MUB + q]; th.wq[q] = out[CCAKE_COL_WB + q]; }
+  th.p = out[CCAKE_COL_P]; th.cs2 = out[CCAKE_COL_CS2]; th.e = out[CCAKE_COL_E]; th.ws = out[CCAKE_COL_WS];
+  return th;
+}
+
+/* single real root of 4 c4 mu^3 + 2 c2 T^2 mu = n: depressed cubic chi^3 + a1 chi - a2 = 0, closed form of
+   Eq. A.13-A.14 (:2146-2152) */
+__device__ inline double mu_of_T(const KParams& kp, double T, double n) {
+  if (n == 0.0) return 0.0;
+  if (kp.c4 == 0.0) return n / (2.0 * kp.c2 * T * T);
+  const double sgn = (n < 0.0) ? -1.0 : 1.0;
+  const double a1 = kp.c2 * T * T / (2.0 * kp.c4);
+  const double a2 = fabs(n) / (4.0 * kp.c4);
+  const double delta = sqrt(12.0 * a1 * a1 * a1 + 81.0 * a2 * a2) + 9.0 * a2;
+  const double d13 = cbrt(delta);
+  const double chi = (1.2599210498948732 * d13 * d13 - 2.0 * 1.4422495703074083 * a1) / (3.3019272488946263 * d13);
+  return sgn * chi;
+}
+
+/* (s, n_q) -> (T, mu_q): cubic for mu_q(T), monotone 1-D solve in T by bisection (analogue of Eq. A.15 with s as
+   the key, :587); then p, e = 3p, c_s^2 = 1/3 and dw/ds, dw/dn_q from the Hessian of p (Eq. A.8-A.10) */
+__device__ inline ThermoOut eos_closed_form(const KParams& kp, double s, const double n[NQ]) {
+  ThermoOut th;
+  th.oob = 0;
+  double T;
+  const double Tmax = cbrt(s / (4.0 * kp.c0));
+  if (n[0] == 0.0 && n[1] == 0.0 && n[2] == 0.0) {
+    T = Tmax;
+  } else {
+    double lo = 0.0, hi = Tmax;
+    for (int it = 0; it < 200; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      if (mid <= lo || mid >= hi) break;
+      double m2 = 0.0;
+      for (int q = 0; q < NQ; ++q) { const double m = mu_of_T(kp, mid, n[q]); m2 += m * m; }
+      const double f = 4.0 * kp.c0 * mid * mid * mid + 2.0 * kp.c2 * mid * m2 - s;
+      if (f > 0.0) hi = mid; else lo = mid;
+    }
+    T = 0.5 * (lo + hi);
+  }
+  th.T = T;
+  double m2 = 0.0, m4 = 0.0;
+  for (int q = 0; q < NQ; ++q) {
+    const double m = mu_of_T(kp, T, n[q]);
+    th.mu[q] = m;
+    m2 += m * m;
+    m4 += m * m * m * m;
+  }
+  th.p = kp.c0 * T * T * T * T + kp.c2 * T * T * m2 + kp.c4 * m4;
+  th.e = 3.0 * th.p;
+  th.cs2 = 1.0 / 3.0;
+  /* H = Hessian of p in (T, mu): arrow matrix [[a, b^T], [b, diag(d)]]; z = H^-1 (s, n) by the Schur complement;
+     dw/ds = T + z_0, dw/dn_q = mu_q + z_q */
+  const double a = 12.0 * kp.c0 * T * T + 2.0 * kp.c2 * m2;
+  double b[NQ], d[NQ];
+  bool ok = true;
+  for (int q = 0; q < NQ; ++q) {
+    b[q] = 4.0 * kp.c2 * T * th.mu[q];
+    d[q] = 2.0 * kp.c2 * T * T + 12.0 * kp.c4 * th.mu[q] * th.mu[q];
+    if (d[q] == 0.0) ok = false;
+  }
+  if (ok) {
+    double schur = a, rhs0 = s;
+    for (int q = 0; q < NQ; ++q) { schur -= b[q] * b[q] / d[q]; rhs0 -= b[q] * n[q] / d[q]; }
+    const double z0 = rhs0 / schur;
+    th.ws = T + z0;
+    for (int q = 0; q < NQ; ++q) th.wq[q] = th.mu[q] + (n[q] - b[q] * z0) / d[q];
+  } else {               /* c2 = 0 and mu = 0: charges decouple */
+    th.ws = T + T / 3.0;
+    for (int q = 0; q < NQ; ++q) th.wq[q] = 0.0;
+  }
+  return th;
+}
+
+/* dissipative tensors of one particle: evolved spatial components from the store, time components from
+   u_mu pi^{mu nu} = 0 and u_mu J^mu = 0 (never evolved; DESIGN reading 13) */
+struct Dissip { double pit[4][4], Jt[NQ][4], bulkt; };
+
+__device__ inline void load_dissip(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad,
+                                   int64_t a, const double u[4], Dissip& ds) {
+  const int D = kp.D;
+  const double gam = u[0];
+  const double G[4] = {0.0, 1.0, 1.0, gm.G3};
+  for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) ds.pit[m][n] = 0.0;
+  for (int q = 0; q < NQ; ++q) for (int m = 0; m < 4; ++m) ds.Jt[q][m] = 0.0;
+  ds.bulkt = kp.bulk ? Y[CCAKE_BULK * npad + a] : 0.0;
+  if (kp.shear) {
+    ds.pit[1][1] = Y[CCAKE_PI11 * npad + a];
+    ds.pit[1][2] = ds.pit[2][1] = Y[CCAKE_PI12 * npad + a];
+    ds.pit[2][2] = Y[CCAKE_PI22 * npad + a];
+    ds.pit[3][3] = Y[CCAKE_PI33 * npad + a];
+    if (D == 3) {
+      ds.pit[1][3] = ds.pit[3][1] = Y[CCAKE_PI13 * npad + a];
+      ds.pit[2][3] = ds.pit[3][2] = Y[CCAKE_PI23 * npad + a];
+    }
+    for (int i = 1; i <= 3; ++i) {
+      double acc = 0.0;
+      for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.pit[j][i];
+      ds.pit[0][i] = ds.pit[i][0] = acc / gam;
+    }
+    double acc = 0.0;
+    for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.pit[j][0];
+    ds.pit[0][0] = acc / gam;
+  }
+  if (kp.diff) {
+    for (int q = 0; q < NQ; ++q) {
+      for (int i = 1; i <= D; ++i) ds.Jt[q][i] = Y[(CCAKE_JB1 + 3 * q + (i - 1)) * npad + a];
+      double acc = 0.0;
+      for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.Jt[q][j];
+      ds.Jt[q][0] = acc / gam;
+    }
+  }
+}
+
+__device__ inline void load_u(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad, int64_t a,
+                              double u[4]) {
+  u[1] = Y[CCAKE_U1 * npad + a];
+  u[2] = Y[CCAKE_U2 * npad + a];
+  u[3] = (kp.D == 3) ? Y[CCAKE_U3 * npad + a] : 0.0;
+  u[0] = sqrt(1.0 + u[1] * u[1] + u[2] * u[2] + gm.G3 * u[3] * u[3]);
+}
+
+__global__ void __launch_bounds__(128)
+thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restrict__ Y, int64_t npad, Sorted so,
+              Status* __restrict__ status) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int D = kp.D;
+  const int64_t a = so.perm[i];
+  double u[4];
+  load_u(kp, gm, Y, npad, a, u);
+  const double gam = u[0];
+  const double lab = gam * gm.sqrtg;
+  const double sst = so.sigma_star[i];
+  const double sig = sst / lab, s = so.s_star[i] / lab;
+  double nq[NQ];
+  for (int q = 0; q < NQ; ++q) nq[q] = so.rho_star[q][i] / lab;
+  const ThermoOut th = (kp.eos_kind == 0) ? eos_closed_form(kp, s, nq) : eos_table_lookup(tb, s, nq);
+  if (th.oob) atomicAdd(&status->n_oob, 1ULL);
+  so.gamma[i] = gam; so.sigma[i] = sig; so.s[i] = s;
+  so.T[i] = th.T; so.p[i] = th.p; so.e[i] = th.e; so.cs2[i] = th.cs2; so.ws[i] = th.ws;
+  for (int q = 0; q < NQ; ++q) {
+    so.n[q][i] = nq[q]; so.mu[q][i] = th.mu[q]; so.wq[q][i] = th.wq[q];
+    so.alpha[q][i] = th.mu[q] / th.T;
+  }
+  Dissip ds;
+  load_dissip(kp, gm, Y, npad, a, u, ds);
+  const double sst2 = sst * sst;
+  const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
+  so.Ppair[i] = (th.p + ds.bulkt * sig) / sst2;
+  for (int j = 1; j <= 3; ++j) {
+    so.u[j - 1][i] = u[j];
+    so.v[j - 1][i] = (j <= D) ? u[j] / gam : 0.0;
+  }
+  if (kp.shear)
+    for (int j = 1; j <= D; ++j)
+      for (int k = 1; k <= D; ++k) {
+        const double pi_j_k = sig * ds.pit[j][k] * glo[k];
+        const double pi_0_k = sig * ds.pit[0][k] * glo[k];
+        so.Bpair[(j - 1) * 3 + (k - 1)][i] = (pi_j_k - (u[j] / gam) * pi_0_k) / sst2;
+      }
+  if (kp.diff)
+    for (int q = 0; q < NQ; ++q)
+      for (int j = 1; j <= D; ++j)
+        so.Kpair[q * 3 + (j - 1)][i] = (sig * ds.Jt[q][j] - (u[j] / gam) * sig * ds.Jt[q][0]) / sst2;
+}
+
+}  // namespace ccake
