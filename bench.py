@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the SPH hot path (libccake, C ABI) on B200, with the oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+
+A "step" is one full RK step (ccake_step(ctx, 1)): every row a1-a8 of SURVEY.md §8(a) twice (RK2 midpoint) over
+one batch of synthetic particles; row a9 (conserved totals) closes the run.  The default workload is BASELINE.json's
+config 4 ("C4": (3+1)D viscous, DNMR shear + bulk + BSQ diffusion, 1,984,000 particles in 10 seeded event tiles,
+100x32^3 EoS table with 11 columns) — the configuration `north_star` quotes its target on.  State (416 MB) and work
+arrays are far larger than the 126 MB L2, so consecutive steps see cold data ("inputs larger than L2").
+
+N > 1 (torchrun): the path shards by independent event tiles with no data-path collective — every rank runs its
+own batch of tiles (different seeds), "scaling": "weak"; the only collectives are the barrier and the max-over-ranks
+of the device time (NCCL).
+
+One JSON line on stdout (rank 0).  DESIGN.md §"Measurement" defines every figure.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "SPH particle-updates/s (fp64)"
+UNIT = "particle-updates/s"
+
+# algorithmic work per unit (DESIGN.md §"Algorithmic work")
+FLOP_SMOOTH_PER_PAIR = 35.0
+
+
+def flop_grad_per_pair(D, visc, diff):
+    terms = D + D * D + D          # FP, DU, div v
+    if visc:
+        terms += D * D             # FB
+    if diff:
+        terms += 6 * D             # grad alpha_q, FK_q
+    return 34.0 + 3.0 * terms
+
+
+FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
+
+
+def make_workload(name, rank=0, small=False):
+    from paper_2511_22852_b200 import workloads as W
+    if name == "C1":
+        return W.config_c1()
+    if name == "C2":
+        return W.config_c2()
+    if name == "C3":
+        return W.config_c3(tile0=4 * rank)
+    if name == "C4":
+        if small:
+            return W.config_c4(K=1, tile0=10 * rank)
+        return W.config_c4(tile0=10 * rank)
+    if name == "C5":
+        return W.config_c5(tile0=13 * rank)
+    raise SystemExit(f"unknown config {name}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device):
+        self.path = tempfile.mktemp(suffix=".csv")
+        self.proc = None
+        try:
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(device), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.fh,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.fh.close()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            with open(self.path) as fh:
+                for line in fh:
+                    f = [x.strip() for x in line.split(",")]
+                    if len(f) < 9:
+                        continue
+                    try:
+                        sm.append(float(f[1])); smax.append(float(f[2]))
+                    except ValueError:
+                        continue
+                    for nm, v in zip(names, f[5:9]):
+                        if v.lower().startswith("active"):
+                            reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "reasons": sorted(reasons),
+                   "samples": len(sm)}
+        return out
+
+
+def oracle_sample(name):
+    """Bounded sample of the workload for the CPU oracle: one event tile of the tiled configs (the tiles are
+    independent events separated by gaps > 2h, so one tile is a faithful 1/K sample); whole workload for C1, C2."""
+    from paper_2511_22852_b200 import workloads as W
+    if name == "C3":
+        return W.config_c3(K=1), "1 of 4 event tiles (54,289 particles), 1 RK2 step"
+    if name == "C4":
+        return W.config_c4(K=1), "1 of 10 event tiles (198,400 particles), 1 RK2 step"
+    if name == "C5":
+        return W.config_c5(K=1, n_eta=5), "1 of 13 event tiles cut to 5 rapidity slices (353,780 particles), 1 RK2 step"
+    w = make_workload(name)
+    return w, f"whole workload ({w.n} particles), 1 RK2 step"
+
+
+def time_oracle(name, steps, warmup):
+    """The oracle as it stands, on this host's cores; returns (updates/s, ms per step, cores, sample text)."""
+    import oracle as O
+    w, what = oracle_sample(name)
+    o = O.Oracle(**w.params)
+    if w.table is not None:
+        o.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], w.table["data"])
+    o.load_particles(w.fields)
+    for _ in range(warmup):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(1)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return w.n * steps / dt, 1e3 * dt / steps, cores, what, w
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 3))
+    val, ms, cores, what, w = time_oracle(args.config, steps, 0 if args.config in ("C4", "C5") else min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_text(args.config), "sample": what},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_text(name):
+    return {
+        "C1": "BASELINE.json configs[0]: (2+1)D ideal Cartesian, 2,500 particles, closed-form EoS, RK2",
+        "C2": "BASELINE.json configs[1]: (2+1)D ideal BSQ Gubser, hyperbolic, 40,000 particles, table 100x32^3x8, RK2",
+        "C3": "BASELINE.json configs[2]: (2+1)D viscous hyperbolic, 217,156 particles (4 event tiles), IS shear+bulk+diffusion, table 100x32^3x11, RK2",
+        "C4": "BASELINE.json configs[3]: (3+1)D viscous hyperbolic, 1,984,000 particles (10 event tiles of 80x80x31), DNMR shear+bulk+BSQ diffusion, table 100x32^3x11, h=0.3, RK2",
+        "C5": "BASELINE.json configs[4]: (3+1)D viscous hyperbolic, 19,316,388 particles (13 event tiles of 266x266x21), IS shear+bulk+diffusion, table 200x48^3x11, RK2",
+    }[name]
+
+
+def algorithmic_bytes_per_particle(D, visc, bulk, diff, ncols):
+    """HBM bytes each kernel group must move per particle per substep: 8 B x (fields read once + written once);
+    a neighbour's data counts once (DESIGN.md §"Algorithmic work").  Returns dict per group."""
+    n_pi = (6 if D == 3 else 4) if visc else 0
+    n_J = 3 * D if diff else 0
+    n_state = 2 * D + 4 + (1 if bulk else 0) + n_pi + n_J
+    sort = 8 * D + 4 * 2 * 2 * 3            # read r; 3 radix passes each read+write (key, value) u32
+    smooth = 8 * (D + 5 + 5)                # read r, S, N_q, m; write 5 sums
+    n_pair_in = 1 + D + D + (D * D if visc else 0) + (n_J + 3 if diff else 0)      # P, u, v, B, K, alpha
+    thermo = 8 * (5 + D + (1 if bulk else 0) + n_pi + n_J) + 8 * (8 + 3 + n_pair_in)
+    gather = 16 * ncols * 8
+    n_grad_out = 2 * D + D * D + 1 + (3 * D + 3 if diff else 0)
+    grad = 8 * (D + n_pair_in + n_grad_out)
+    eom = 8 * (n_grad_out + 14 + 2 * n_state + n_state)    # sums, thermo, y_cur, y_base; write y_out
+    return {"sort": sort, "smooth": smooth, "thermo": thermo + gather, "grad": grad, "eom": eom}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2511_22852_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()   # fails loudly when libccake.so is missing
+
+    w = make_workload(args.config, rank=rank)
+    p = w.params
+    D = p["dim"]
+    visc, bulk, diff = bool(p["flags"] & 1) and p["eom"] != 0, bool(p["flags"] & 2) and p["eom"] != 0, bool(p["flags"] & 4) and p["eom"] != 0
+    stream = torch.cuda.Stream()
+    sim = B.Ccake(device=local, stream=stream.cuda_stream, **p)
+    dev = torch.device("cuda", local)
+    if w.table is not None:
+        sim.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"],
+                           torch.as_tensor(w.table["data"], device=dev))
+    ids = list(w.fields.keys())
+    dfields = {k: torch.as_tensor(np.ascontiguousarray(w.fields[k]), device=dev) for k in ids}
+    sim.load_particles(dfields)
+    npairs = float(sim.conserved_totals()[14])          # ordered neighbour pairs, excluding self
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -----------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        sim.step(1)
+    sim.synchronize(strict=False)
+    sim.load_particles(dfields)       # timed steps start from the loaded state, inputs resident in HBM
+    sim.enable_timing(True)
+    sim.launch_count()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record()
+        for _ in range(args.steps):
+            sim.step(1)
+        e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_total = e0.elapsed_time(e1)
+    launches = sim.launch_count()
+    kt = sim.kernel_times()           # per-substep averages of each kernel group, CUDA events on the same stream
+    sim.enable_timing(False)
+    rc = sim.synchronize(strict=False)
+    from paper_2511_22852_b200 import sharding
+    ms_total = sharding.reduce_max(ms_total, dev)                 # max over ranks of the device time
+    tot_n = torch.tensor([float(w.n)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tot_n, op=dist.ReduceOp.SUM)
+    n_all = float(tot_n.item())
+    value = n_all * args.steps / (ms_total * 1e-3)
+    totals = sim.conserved_totals()
+
+    # ---- end to end through the C ABI with HOST buffers -----------------------------------------------------
+    host_in = {k: torch.empty(w.n, dtype=torch.float64).pin_memory() for k in ids}
+    for k in ids:
+        host_in[k].numpy()[:] = w.fields[k]
+    out_ids = B.state_field_ids(p)
+    host_out = [torch.empty(w.n, dtype=torch.float64).pin_memory() for _ in out_ids]
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.load_particles({k: host_in[k] for k in ids})       # H2D inside the timed region
+        sim.step(1)
+        sim.read_fields(out_ids, out=host_out)                  # D2H inside the timed region (synchronises)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    e2e_value = n_all * e2e_steps / sharding.reduce_max(dt, dev)
+    h2d = 8 * w.n * len(ids)
+    d2h = 8 * w.n * len(out_ids)
+
+    if rank == 0:
+        hbm, which = peaks()
+        nsub = 2 if p["integrator"] == 2 else 4
+        ncols = len(w.table["col_ids"]) if w.table is not None else 0
+        bytes_pp = algorithmic_bytes_per_particle(D, visc, bulk, diff, ncols)
+        names = ["sort", "pack", "smooth", "thermo", "grad", "eom"]
+        groups = {nm: float(kt[i]) for i, nm in enumerate(names)}
+        fg = flop_grad_per_pair(D, visc, diff)
+        dom = max(("smooth", "grad"), key=lambda k: groups[k])
+        flop = npairs * (fg if dom == "grad" else FLOP_SMOOTH_PER_PAIR)
+        ach = flop / (groups[dom] * 1e-3) / 1e12 if groups[dom] > 0 else 0.0
+        kernels = {}
+        for nm in names:
+            if nm == "pack" or groups[nm] <= 0:
+                continue
+            b = bytes_pp[nm] * w.n
+            kernels[nm] = {"ms": groups[nm], "alg_GB": b / 1e9, "GBps": b / (groups[nm] * 1e-3) / 1e9,
+                           "hbm_frac": b / (groups[nm] * 1e-3) / 1e9 / hbm}
+        kernels["smooth"]["TFLOPs"] = npairs * FLOP_SMOOTH_PER_PAIR / (groups["smooth"] * 1e-3) / 1e12
+        kernels["grad"]["TFLOPs"] = npairs * fg / (groups["grad"] * 1e-3) / 1e12
+        total_bytes = sum(bytes_pp.values()) * w.n
+        cpu_val, cpu_ms, cores, what, _ = time_oracle(args.config, 1, 0) if not args.no_cpu else (None, None, 0, "skipped", None)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_text(args.config), "particles_per_gpu": w.n, "rk_substeps_per_step": nsub,
+                       "ordered_pairs_per_pass": npairs, "l2": "inputs larger than L2 (state + work arrays > 1 GB per substep)"},
+            "pair_interactions_per_s": npairs * 2 * nsub * args.steps * world / (ms_total * 1e-3),
+            "substep_hbm_frac": total_bytes * nsub / (ms_total / args.steps * 1e-3) / 1e9 / hbm,
+            "roofline": {"bound": "alu", "kernel": {"grad": "gradient pass a6", "smooth": "smoothing pass a4"}[dom],
+                         "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
+                         "traffic": None, "peak_source": "fp64 DFMA: 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "flop_per_pair": fg if dom == "grad" else FLOP_SMOOTH_PER_PAIR,
+                         "hbm_peak_GBps": hbm, "hbm_peak_source": which},
+            "kernels": kernels,
+            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
+                             "ms_per_step": cpu_ms},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps},
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "status": {"rc": rc, "n_out_of_table": totals[11], "n_bad": totals[13], "x0": totals[0]},
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

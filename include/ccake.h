@@ -139,6 +139,10 @@ int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity);
 int ccake_kernel_times(ccake_ctx* c, double out[8]);
 int ccake_enable_timing(ccake_ctx* c, int32_t on);
 
+/* Measurement hook: *out = number of CUDA kernels this context enqueued since the previous call (host counter,
+ * no synchronisation); the counter is then reset. */
+int ccake_launch_count(ccake_ctx* c, int64_t* out);
+
 const char* ccake_last_error(const ccake_ctx* c);
 
 #ifdef __cplusplus

@@ -30,7 +30,8 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
-           "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_last_error"]
+           "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
+           "ccake_last_error"]
 
 
 class Params(C.Structure):
@@ -77,6 +78,7 @@ def lib():
         L.ccake_neighbor_hash.argtypes = [vp, vp, i64]
         L.ccake_kernel_times.argtypes = [vp, C.POINTER(C.c_double)]
         L.ccake_enable_timing.argtypes = [vp, i32]
+        L.ccake_launch_count.argtypes = [vp, C.POINTER(i64)]
         L.ccake_last_error.argtypes = [vp]
         L.ccake_last_error.restype = C.c_char_p
         _lib = L
@@ -215,10 +217,29 @@ class Ccake:
     def enable_timing(self, on=True):
         self._chk(lib().ccake_enable_timing(self._h, 1 if on else 0), "ccake_enable_timing")
 
+    def launch_count(self):
+        out = C.c_int64(0)
+        self._chk(lib().ccake_launch_count(self._h, C.byref(out)), "ccake_launch_count")
+        return int(out.value)
+
     def kernel_times(self):
         out = (C.c_double * 8)()
         self._chk(lib().ccake_kernel_times(self._h, out), "ccake_kernel_times")
         return np.array(out[:], dtype=np.float64)
+
+
+def state_field_ids(params: dict):
+    """Ids of the evolved state fields for a parameter set (what ccake_step advances)."""
+    D = params["dim"]
+    fl = params["flags"] if params["eom"] != 0 else 0
+    ids = [R1, R2] + ([R3] if D == 3 else []) + [U1, U2] + ([U3] if D == 3 else []) + [S, NB, NS, NQ]
+    if fl & 2:
+        ids.append(BULK)
+    if fl & 1:
+        ids += [PI11, PI12, PI22, PI33] + ([PI13, PI23] if D == 3 else [])
+    if fl & 4:
+        ids += [JB1 + 3 * q + j for q in range(3) for j in range(D)]
+    return ids
 
 
 def from_workload(w, device=0, stream=None, memspace="host") -> Ccake:

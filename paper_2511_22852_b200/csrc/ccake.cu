@@ -67,6 +67,8 @@ struct ccake_ctx {
   size_t ev_used = 0;
   int64_t substeps_timed = 0;
 
+  int64_t launches = 0;   /* kernels enqueued since the last ccake_launch_count() */
+
   std::string err;
 };
 
@@ -196,7 +198,9 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
     std::swap(c->orig[0], c->orig[1]);
     Ycur = c->Y[0];
     iota_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.perm, N);
+    c->launches += 2;
   }
+  c->launches += 4 + 4 * c->passes;
   return launch_check(c, "build_cells");
 }
 
@@ -232,6 +236,7 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   rk.theta_out = c->theta;
   eom_kernel<D><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
   if ((rc = mark(c))) return rc;
+  c->launches += 5;
   return launch_check(c, "substep");
 }
 
@@ -485,6 +490,25 @@ int ccake_destroy(ccake_ctx* c) {
   return CCAKE_OK;
 }
 
+/* same particle count as the resident set: keep every allocation, overwrite the state, reset time and status */
+static int reload_particles(ccake_ctx* c, int32_t nfields, const int32_t* ids, const double* const* cols, int32_t memspace) {
+  const int64_t n = c->N, np = c->npad;
+  CK(cudaMemsetAsync(c->Y[0], 0, sizeof(double) * np * NSTATE, c->stream));
+  fill_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->Y[0] + (int64_t)CCAKE_MASS * np, n, 1.0);
+  for (int k = 0; k < nfields; ++k) {
+    const int f = ids[k];
+    if (!((c->field_mask & (1u << f)) || f == CCAKE_MASS)) continue;
+    CK(cudaMemcpyAsync(c->Y[0] + (int64_t)f * np, cols[k], sizeof(double) * n,
+                       memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
+  }
+  iota_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->orig[0], n);
+  CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
+  c->launches += 2;
+  c->x0 = c->P.x0_start;
+  c->derived_valid = false;
+  return launch_check(c, "reload");
+}
+
 int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* ids, const double* const* cols,
                          int32_t memspace) {
   if (!c) return CCAKE_EINVAL;
@@ -496,6 +520,7 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
     if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in load"; return CCAKE_EINVAL; }
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->stream));
+  if (c->loaded && n == c->N) return reload_particles(c, nfields, ids, cols, memspace);
   free_particles(c);
   c->N = n;
   c->npad = (n + 31) / 32 * 32;
@@ -801,6 +826,14 @@ int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   cudaFree(d);
   if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return CCAKE_ECUDA; }
+  return CCAKE_OK;
+}
+
+int ccake_launch_count(ccake_ctx* c, int64_t* out) {
+  if (!c) return CCAKE_EINVAL;
+  if (!out) { c->err = "null out"; return CCAKE_EINVAL; }
+  *out = c->launches;
+  c->launches = 0;
   return CCAKE_OK;
 }
 

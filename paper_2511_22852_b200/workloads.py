@@ -281,7 +281,7 @@ def _event_tile(seed, tile, n_side, dx, n_hot, width, R, a, eta_nodes=None, stop
 
 
 def _tiled_event(name, cfg_index, K, n_side, dx, n_hot, width, R, a, params, nsteps, eta_nodes=None,
-                 stopping=False, table=None):
+                 stopping=False, table=None, tile0=0):
     h = params["h"]
     gap = 2.0 * h + 2.0 * nsteps * params["dx0"]
     box = n_side * dx
@@ -290,7 +290,7 @@ def _tiled_event(name, cfg_index, K, n_side, dx, n_hot, width, R, a, params, nst
     tau0 = params["x0_start"] if params["coords"] == 1 else 1.0
     dV = dx * dx * ((eta_nodes[1] - eta_nodes[0]) if eta_nodes is not None else 1.0)
     for t in range(K):
-        x, y, e, s, rho = _event_tile(SEED0 + cfg_index, t, n_side, dx, n_hot, width, R, a, eta_nodes, stopping)
+        x, y, e, s, rho = _event_tile(SEED0 + cfg_index, tile0 + t, n_side, dx, n_hot, width, R, a, eta_nodes, stopping)
         ox = (t % wide) * (box + gap)
         oy = (t // wide) * (box + gap)
         cols[R1].append(x + ox); cols[R2].append(y + oy)
@@ -311,31 +311,32 @@ def viscous_params(dim, eom, dx0, x0=0.6):
                        kappa_over_T2=list(KAPPA_OVER_T2), tau_q_times_T=list(TAU_Q_TIMES_T))
 
 
-def config_c3(K=4, n_side=233, nsteps=100, n_hot=200, table=None):
+def config_c3(K=4, n_side=233, nsteps=100, n_hot=200, table=None, tile0=0):
     """C3: (2+1)D viscous Pb+Pb-like event tiles, minimal IS shear + bulk + BSQ diffusion, 11-column table."""
     params = viscous_params(2, 1, 0.025)
     if table is None:
         table = make_eos_table(100, 32, with_wq=True)
-    return _tiled_event("C3", 3, K, n_side, 0.06, n_hot, 0.5, 6.6, 0.45, params, nsteps, table=table)
+    return _tiled_event("C3", 3, K, n_side, 0.06, n_hot, 0.5, 6.6, 0.45, params, nsteps, table=table, tile0=tile0)
 
 
-def config_c4(K=10, n_side=80, n_eta=31, nsteps=50, n_hot=40, table=None):
+def config_c4(K=10, n_side=80, n_eta=31, nsteps=50, n_hot=40, table=None, tile0=0):
     """C4: (3+1)D viscous O+O-like event tiles, DNMR shear + bulk + diffusion, 11-column table."""
     params = viscous_params(3, 2, 0.05)
     eta = (np.arange(n_eta) - 0.5 * (n_eta - 1)) * 0.1
     if table is None:
         table = make_eos_table(100, 32, with_wq=True)
-    return _tiled_event("C4", 4, K, n_side, 0.1, n_hot, 0.4, 2.6, 0.513, params, nsteps, eta_nodes=eta, table=table)
+    return _tiled_event("C4", 4, K, n_side, 0.1, n_hot, 0.4, 2.6, 0.513, params, nsteps, eta_nodes=eta, table=table,
+                        tile0=tile0)
 
 
-def config_c5(K=13, n_side=266, n_eta=21, nsteps=20, n_hot=400, table=None, ns=200, nq=48):
+def config_c5(K=13, n_side=266, n_eta=21, nsteps=20, n_hot=400, table=None, ns=200, nq=48, tile0=0):
     """C5: (3+1)D high-resolution Au+Au-like event tiles with baryon stopping, minimal IS, 200x48^3 table."""
     params = viscous_params(3, 1, 0.025)
     eta = (np.arange(n_eta) - 0.5 * (n_eta - 1)) * 0.15
     if table is None:
         table = make_eos_table(ns, nq, with_wq=True)
     return _tiled_event("C5", 5, K, n_side, 0.06, n_hot, 0.5, 6.4, 0.54, params, nsteps, eta_nodes=eta,
-                        stopping=True, table=table)
+                        stopping=True, table=table, tile0=tile0)
 
 
 def count_pairs_estimate(w: Workload) -> float:
