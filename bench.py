@@ -50,7 +50,7 @@ def flop_grad_per_pair(D, visc, diff):
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 
 
-def make_workload(name, rank=0, small=False):
+def make_workload(name, rank=0, tiles=None):
     from paper_2511_22852_b200 import workloads as W
     if name == "C1":
         return W.config_c1()
@@ -59,9 +59,7 @@ def make_workload(name, rank=0, small=False):
     if name == "C3":
         return W.config_c3(tile0=4 * rank)
     if name == "C4":
-        if small:
-            return W.config_c4(K=1, tile0=10 * rank)
-        return W.config_c4(tile0=10 * rank)
+        return W.config_c4(K=tiles or 10, tile0=10 * rank)
     if name == "C5":
         return W.config_c5(tile0=13 * rank)
     raise SystemExit(f"unknown config {name}")
@@ -218,7 +216,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()   # fails loudly when libccake.so is missing
 
-    w = make_workload(args.config, rank=rank)
+    w = make_workload(args.config, rank=rank, tiles=args.tiles)
     p = w.params
     D = p["dim"]
     visc, bulk, diff = bool(p["flags"] & 1) and p["eom"] != 0, bool(p["flags"] & 2) and p["eom"] != 0, bool(p["flags"] & 4) and p["eom"] != 0
@@ -345,6 +343,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--tiles", type=int, default=None, help="C4 only: number of event tiles (profiling runs; default 10)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

@@ -16,7 +16,6 @@
 #include "eom.cuh"
 #include "grid_sort.cuh"
 #include "pair_tiled.cuh"
-#include "pair_v1.cuh"
 #include "thermo_eos.cuh"
 #include "totals.cuh"
 
@@ -35,7 +34,6 @@ struct ccake_ctx {
   bool loaded = false, table_loaded = false, derived_valid = false;
   double x0 = 0.0;
   uint32_t field_mask = 0;
-  int pair_impl = 0;    /* 0 tiled kernels, 1 thread-per-particle v1 */
 
   double* Y[3] = {nullptr, nullptr, nullptr};   /* Y0, stage, RK4 accumulator */
   double* Krate = nullptr;
@@ -56,7 +54,6 @@ struct ccake_ctx {
   double* theta = nullptr;
   double* scratch = nullptr;    /* N doubles: read_fields staging */
   Sorted so;
-  PairWork pw;
 
   TableDev tb;
   double* tb_axes = nullptr;
@@ -103,7 +100,6 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->nnb); c->nnb = nullptr;
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
-  pair_work_free(c->pw);
   c->loaded = false;
 }
 
@@ -124,18 +120,17 @@ int mark(ccake_ctx* c) {
   return CCAKE_OK;
 }
 
-/* layout of the sorted-order arena */
-constexpr int ARENA_FIELDS = 3 + 1 + 3 + 1 + 5 + 6 + 11 + 1 + 9 + 9 + 3 + 3 + 3 + 3 + 3 + 3 + 9 + 9 + 1;
+/* layout of the sorted-order arena, in units of npad doubles */
+constexpr int ARENA_FIELDS = 3 + 2 + 8 + 5 + 6 + 11 + 32 + 3 + 3 + 3 + 9 + 9 + 1;
 
 void carve(ccake_ctx* c) {
   Sorted& s = c->so;
   double* p = c->arena;
   const int64_t np = c->npad;
-  auto take = [&]() { double* r = p; p += np; return r; };
+  auto take = [&](int k = 1) { double* r = p; p += np * k; return r; };
   for (int k = 0; k < 3; ++k) s.x[k] = take();
-  s.S = take();
-  for (int q = 0; q < NQ; ++q) s.Nq[q] = take();
-  s.m = take();
+  s.xf = reinterpret_cast<float4*>(take(2));
+  s.rec_s = take(8);
   s.sigma_star = take(); s.s_star = take();
   for (int q = 0; q < NQ; ++q) s.rho_star[q] = take();
   s.gamma = take(); s.sigma = take(); s.s = take();
@@ -144,12 +139,7 @@ void carve(ccake_ctx* c) {
   for (int q = 0; q < NQ; ++q) s.mu[q] = take();
   s.p = take(); s.e = take(); s.cs2 = take(); s.ws = take();
   for (int q = 0; q < NQ; ++q) s.wq[q] = take();
-  s.Ppair = take();
-  for (int k = 0; k < 9; ++k) s.Bpair[k] = take();
-  for (int k = 0; k < 9; ++k) s.Kpair[k] = take();
-  for (int q = 0; q < NQ; ++q) s.alpha[q] = take();
-  for (int k = 0; k < 3; ++k) s.v[k] = take();
-  for (int k = 0; k < 3; ++k) s.u[k] = take();
+  s.rec_g = take(32);
   for (int k = 0; k < 3; ++k) s.FP[k] = take();
   for (int k = 0; k < 3; ++k) s.FB[k] = take();
   for (int q = 0; q < NQ; ++q) s.FK[q] = take();
@@ -211,24 +201,17 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   const KParams& kp = c->kp;
   const Geom gm = make_geom(c->P.coords, x0s);
   int rc;
-  pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->so);
+  pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->grid, c->so);
   if ((rc = mark(c))) return rc;
   /* a4 */
-  if (c->pair_impl == 1) smoothing_v1_kernel<D><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
-  else if ((rc = launch_smoothing_tiled<D>(c->pw, N, kp, c->grid, c->so, st))) { c->err = "smoothing launch"; return CCAKE_ECUDA; }
+  launch_smoothing<D>(N, kp, c->grid, c->so, st);
   if ((rc = mark(c))) return rc;
   /* a5 */
   cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
   thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, c->tb, Ycur, np, c->so, c->status);
   if ((rc = mark(c))) return rc;
   /* a6 */
-  const bool visc = kp.shear, diff = kp.diff;
-  if (c->pair_impl == 1) {
-    if (visc && diff) gradient_v1_kernel<D, true, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
-    else if (visc) gradient_v1_kernel<D, true, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
-    else if (diff) gradient_v1_kernel<D, false, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
-    else gradient_v1_kernel<D, false, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->grid, c->so);
-  } else if ((rc = launch_gradient_tiled<D>(c->pw, N, kp, c->grid, c->so, visc, diff, st))) { c->err = "gradient launch"; return CCAKE_ECUDA; }
+  launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
   if ((rc = mark(c))) return rc;
   /* a7 + a8 */
   RkArgs rk = rk_in;
@@ -370,7 +353,7 @@ __global__ void neighbour_walk_kernel(int64_t n, KParams kp, const Grid* __restr
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const Grid g = *grid;
-  const uint32_t cid = so.key[i];
+  const uint32_t cid = so.key[i] >> g.mb;
   const int cx = cid % g.nc[0], cy = (cid / g.nc[0]) % g.nc[1], cz = cid / (g.nc[0] * g.nc[1]);
   const double xa = so.x[0][i], ya = so.x[1][i], za = (D == 3) ? so.x[2][i] : 0.0;
   const uint32_t ao = orig[so.perm[i]];
@@ -426,7 +409,6 @@ int ccake_create(const ccake_params* p, ccake_ctx** out) {
   c->x0 = p->x0_start;
   std::memset(&c->so, 0, sizeof(c->so));
   std::memset(&c->tb, 0, sizeof(c->tb));
-  std::memset(&c->pw, 0, sizeof(c->pw));
   if (cudaSetDevice(c->device) != cudaSuccess) { delete c; return CCAKE_ECUDA; }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess || prop.major < 10) {
@@ -465,8 +447,6 @@ int ccake_create(const ccake_params* p, ccake_ctx** out) {
     for (int q = 0; q < 3; ++q) for (int j = 0; j < p->dim; ++j) on(CCAKE_JB1 + 3 * q + j);
   if (p->coords == 1 && p->dim == 2) on(CCAKE_WORK);
   c->field_mask = m;
-  const char* impl = std::getenv("CCAKE_PAIR_IMPL");
-  c->pair_impl = (impl && impl[0] == '1') ? 1 : 0;
   if (cudaMalloc(&c->grid, sizeof(Grid)) != cudaSuccess || cudaMalloc(&c->status, sizeof(Status)) != cudaSuccess) {
     cudaFree(c->grid);
     delete c;
@@ -563,20 +543,21 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
   /* size the radix-sort key from the bounding box at load; the device coarsens the grid if the system outgrows it */
   bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, c->stream>>>(c->Y[0], np, n, c->P.dim, c->bbox_partial);
-  bbox_final_kernel<<<1, 32, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 24, c->grid);
+  bbox_final_kernel<<<1, 32, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 22, c->grid);
   Grid g;
   CK(cudaMemcpyAsync(&g, c->grid, sizeof(Grid), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   {
+    /* room for the system to grow 8x in cell count before the device has to coarsen the grid; the key holds the
+       cell id above g.mb Morton bits and is sorted in 8-bit digits */
     int64_t want = (int64_t)g.ncells * 8;
     int bits = 1;
-    while (((int64_t)1 << bits) < want && bits < 24) ++bits;
-    c->passes = (bits + 7) / 8;
-    c->max_cells = 1 << (8 * c->passes);
+    while (((int64_t)1 << bits) < want && bits < 22) ++bits;
+    c->passes = (bits + g.mb + 7) / 8;
+    c->max_cells = 1 << std::min(22, 8 * c->passes - g.mb);
   }
   CK(cudaMalloc(&c->cell_start, sizeof(uint32_t) * ((size_t)c->max_cells + 2)));
   carve(c);
-  if (pair_work_alloc(c->pw, n, c->max_cells) != 0) { c->err = "pair work allocation failed"; return CCAKE_ENOMEM; }
   c->x0 = c->P.x0_start;
   c->loaded = true;
   c->derived_valid = false;

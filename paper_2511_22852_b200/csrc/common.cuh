@@ -30,6 +30,12 @@ struct Grid {
   /* reported cell id (DESIGN reading 9): edge exactly 2h */
   double rep_inv_edge;
   long long rep_nc[3];
+  /* sort key = (cell id << mb) | Morton code of the position inside the cell (mb bits) */
+  int mb;
+  /* FP32 culling: positions are stored relative to xmin; cutm = 2h + margin covering their rounding, cutm2 its
+     square rounded up */
+  double cutm;
+  float cutm2;
 };
 
 /* geometry of a time slice: g = diag(1, -1, -1, -G3), G3 = tau^2 (hyperbolic) or 1 */
@@ -71,15 +77,17 @@ struct Sorted {
   /* a3 */
   uint32_t *key, *perm;              /* cell id, store slot */
   uint32_t* cell_start;              /* ncells + 1, monotone */
-  /* pack: smoothing payload */
-  double *x[3], *S, *Nq[NQ], *m;
+  /* pack: exact positions (SoA), FP32 positions relative to grid.xmin, AoS payload of the smoothing pass */
+  double* x[3];
+  float4* xf;
+  double* rec_s;      /* [n][8]: x[3], S, N_B, N_S, N_Q, m */
   /* a4 */
   double *sigma_star, *s_star, *rho_star[NQ];
   uint32_t* nnb;
   /* a5 */
   double *gamma, *sigma, *s, *n[NQ];
   double *T, *mu[NQ], *p, *e, *cs2, *ws, *wq[NQ];
-  double *Ppair, *Bpair[9], *Kpair[9], *alpha[NQ], *v[3], *u[3];
+  double* rec_g;      /* [n][NREC]: AoS payload of the gradient pass, layout GLayout (pair_tiled.cuh) */
   /* a6 */
   double *FP[3], *FB[3], *FK[NQ], *DU[9], *DA[9], *divv;
 };

@@ -93,6 +93,14 @@ __global__ void bbox_final_kernel(const double* __restrict__ partial, int nblock
     g.inv_edge = 1.0 / edge;
     g.ncells = g.nc[0] * g.nc[1] * g.nc[2];
     g.rep_inv_edge = 1.0 / twoh;
+    g.mb = (D == 3) ? 9 : 8;
+    {
+      double ext = 0.0;
+      for (int k = 0; k < D; ++k) ext = fmax(ext, g.xmax[k] - g.xmin[k]);
+      if (!(ext < 1.0e300)) ext = 1.0e300;
+      g.cutm = twoh + ext * (1.0 / 1048576.0);                       /* 2^-20 of the extent >> FP32 rounding 2^-24 */
+      g.cutm2 = __double2float_ru(g.cutm * g.cutm * (1.0 + 1.0e-5));
+    }
     for (int k = 0; k < 3; ++k) {
       g.rep_nc[k] = 1;
       if (k < D) g.rep_nc[k] = (long long)floor(__dmul_rn(__dsub_rn(g.xmax[k], g.xmin[k]), g.rep_inv_edge)) + 1;
@@ -109,15 +117,34 @@ __device__ inline int cell_coord(double x, double xmin, double inv_edge, int nc)
   return c;
 }
 
+/* spread the low bits of v so that bit k lands at position k * stride */
+__device__ inline uint32_t spread_bits(uint32_t v, int nbits, int stride) {
+  uint32_t r = 0;
+  for (int k = 0; k < nbits; ++k) r |= ((v >> k) & 1u) << (k * stride);
+  return r;
+}
+
+/* sort key: traversal cell (x fastest) in the high bits; below it the Morton code of the position inside the
+   cell (3 bits per axis in 3-D, 4 in 2-D), so that consecutive particles of a cell form compact clusters */
 __global__ void cell_hash_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
                                  const Grid* __restrict__ grid, uint32_t* __restrict__ key, uint32_t* __restrict__ val) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const Grid g = *grid;
   int c[3] = {0, 0, 0};
+  uint32_t morton = 0;
+  const int sb = g.mb / D;               /* bits per axis */
   for (int k = 0; k < 3; ++k)
-    if (k < D) c[k] = cell_coord(Y[(CCAKE_R1 + k) * npad + i], g.xmin[k], g.inv_edge, g.nc[k]);
-  key[i] = (uint32_t)(c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2]));
+    if (k < D) {
+      const double x = Y[(CCAKE_R1 + k) * npad + i];
+      c[k] = cell_coord(x, g.xmin[k], g.inv_edge, g.nc[k]);
+      const double frac = (x - g.xmin[k]) * g.inv_edge - (double)c[k];
+      int sub = (int)(frac * (double)(1 << sb));
+      sub = max(0, min(sub, (1 << sb) - 1));
+      morton |= spread_bits((uint32_t)sub, sb, D) << k;
+    }
+  const uint32_t cell = (uint32_t)(c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2]));
+  key[i] = (cell << g.mb) | morton;
   val[i] = (uint32_t)i;
 }
 
@@ -262,8 +289,9 @@ __global__ void cell_start_kernel(const uint32_t* __restrict__ key, int64_t n, c
                                   uint32_t* __restrict__ cell_start) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const int64_t k1 = key[i];
-  const int64_t k0 = (i == 0) ? -1 : (int64_t)key[i - 1];
+  const int mb = grid->mb;
+  const int64_t k1 = key[i] >> mb;
+  const int64_t k0 = (i == 0) ? -1 : (int64_t)(key[i - 1] >> mb);
   for (int64_t c = k0 + 1; c <= k1; ++c) cell_start[c] = (uint32_t)i;
   if (i == n - 1) {
     const int ncells = grid->ncells;
@@ -290,20 +318,21 @@ __global__ void iota_kernel(uint32_t* __restrict__ p, int64_t n) {
   if (i < n) p[i] = (uint32_t)i;
 }
 
-/* smoothing payload in sorted order: r, S, N_q, m */
+/* sorted order: exact positions, FP32 positions relative to the grid origin (culling only), and the AoS payload
+   record of the smoothing pass: x[3], S, N_B, N_S, N_Q, m */
 __global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
-                                      const uint32_t* __restrict__ perm, Sorted so) {
+                                      const uint32_t* __restrict__ perm, const Grid* __restrict__ grid, Sorted so) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint32_t a = perm[i];
-  so.x[0][i] = Y[CCAKE_R1 * npad + a];
-  so.x[1][i] = Y[CCAKE_R2 * npad + a];
-  so.x[2][i] = (D == 3) ? Y[CCAKE_R3 * npad + a] : 0.0;
-  so.S[i] = Y[CCAKE_S * npad + a];
-  so.Nq[0][i] = Y[CCAKE_NB * npad + a];
-  so.Nq[1][i] = Y[CCAKE_NS * npad + a];
-  so.Nq[2][i] = Y[CCAKE_NQ * npad + a];
-  so.m[i] = Y[CCAKE_MASS * npad + a];
+  const double x = Y[CCAKE_R1 * npad + a], y = Y[CCAKE_R2 * npad + a], z = (D == 3) ? Y[CCAKE_R3 * npad + a] : 0.0;
+  so.x[0][i] = x; so.x[1][i] = y; so.x[2][i] = z;
+  so.xf[i] = make_float4((float)(x - grid->xmin[0]), (float)(y - grid->xmin[1]), (D == 3) ? (float)(z - grid->xmin[2]) : 0.f, 0.f);
+  double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
+  r[0] = make_double2(x, y);
+  r[1] = make_double2(z, Y[CCAKE_S * npad + a]);
+  r[2] = make_double2(Y[CCAKE_NB * npad + a], Y[CCAKE_NS * npad + a]);
+  r[3] = make_double2(Y[CCAKE_NQ * npad + a], Y[CCAKE_MASS * npad + a]);
 }
 
 }  // namespace ccake
