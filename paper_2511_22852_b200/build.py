@@ -31,7 +31,8 @@ def _deps():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(OUT) and os.path.getmtime(OUT) >= max(os.path.getmtime(p) for p in _deps()):
         return OUT
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT] + sources()
+    extra = os.environ.get("CCAKE_NVCC_EXTRA", "").split()      # experiments only, e.g. -DCCAKE_PAIR_LPS=1
+    cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT] + sources()
     subprocess.run(cmd, check=True)
     return OUT
 

@@ -354,7 +354,8 @@ __global__ void neighbour_walk_kernel(int64_t n, KParams kp, const Grid* __restr
   if (i >= n) return;
   const Grid g = *grid;
   const uint32_t cid = so.key[i] >> g.mb;
-  const int cx = cid % g.nc[0], cy = (cid / g.nc[0]) % g.nc[1], cz = cid / (g.nc[0] * g.nc[1]);
+  int cx, cy, cz;
+  snake_decode(g, cid, cx, cy, cz);
   const double xa = so.x[0][i], ya = so.x[1][i], za = (D == 3) ? so.x[2][i] : 0.0;
   const uint32_t ao = orig[so.perm[i]];
   unsigned long long hsum = 0;
@@ -367,8 +368,9 @@ __global__ void neighbour_walk_kernel(int64_t n, KParams kp, const Grid* __restr
       const int yy = cy + dy;
       if (yy < 0 || yy >= g.nc[1]) continue;
       const int xlo = max(cx - 1, 0), xhi = min(cx + 1, g.nc[0] - 1);
-      const int row = g.nc[0] * (yy + g.nc[1] * zz);
-      const uint32_t b0 = so.cell_start[row + xlo], b1 = so.cell_start[row + xhi + 1];
+      int cfirst, clast;
+      snake_range(g, snake_row(g, yy, zz), xlo, xhi, cfirst, clast);
+      const uint32_t b0 = so.cell_start[cfirst], b1 = so.cell_start[clast + 1];
       for (uint32_t b = b0; b < b1; ++b) {
         if (b == (uint32_t)i) continue;
         const double r2 = dist2_exact(xa - so.x[0][b], ya - so.x[1][b], (D == 3) ? za - so.x[2][b] : 0.0, D);
@@ -549,7 +551,7 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   CK(cudaStreamSynchronize(c->stream));
   {
     /* room for the system to grow 8x in cell count before the device has to coarsen the grid; the key holds the
-       cell id above g.mb Morton bits and is sorted in 8-bit digits */
+       cell id above g.mb Hilbert-index bits and is sorted in 8-bit digits */
     int64_t want = (int64_t)g.ncells * 8;
     int bits = 1;
     while (((int64_t)1 << bits) < want && bits < 22) ++bits;
@@ -851,3 +853,14 @@ int ccake_kernel_times(ccake_ctx* c, double out[8]) {
 }
 
 }  /* extern "C" */
+
+#ifdef CCAKE_PAIR_PROF
+/* experiment builds only (not declared in include/ccake.h): read and clear the section clocks of the pair kernels */
+extern "C" int ccake_debug_pair_prof(unsigned long long out[16]) {
+  unsigned long long z[16] = {0};
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, ccake::g_pair_prof, sizeof(z));
+  cudaMemcpyToSymbol(ccake::g_pair_prof, z, sizeof(z));
+  return 0;
+}
+#endif

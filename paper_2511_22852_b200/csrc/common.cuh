@@ -30,13 +30,37 @@ struct Grid {
   /* reported cell id (DESIGN reading 9): edge exactly 2h */
   double rep_inv_edge;
   long long rep_nc[3];
-  /* sort key = (cell id << mb) | Morton code of the position inside the cell (mb bits) */
+  /* sort key = (cell id << mb) | Hilbert index of the position inside the cell (mb bits) */
   int mb;
   /* FP32 culling: positions are stored relative to xmin; cutm = 2h + margin covering their rounding, cutm2 its
      square rounded up */
   double cutm;
   float cutm2;
 };
+
+/* Cell numbering ("snake"): rows of cells along x are numbered row = y' + nc[1] * z with y' running backwards in
+   odd z-planes, and the cells of an odd row run backwards in x, so that consecutive cell ids are always face
+   neighbours.  Together with the Hilbert index inside the cell (mirrored in x in odd rows) the sorted order is one
+   continuous curve through the occupied space: every run of consecutive particles is spatially compact, also
+   across cell and row ends.  Cells of one row are still contiguous in id, which is all the traversal needs. */
+__host__ __device__ inline int snake_row(const Grid& g, int cy, int cz) {
+  return ((cz & 1) ? g.nc[1] - 1 - cy : cy) + g.nc[1] * cz;
+}
+/* ids of the first and last cell of the physical x-range [x0, x1] of row `row` (first <= last) */
+__host__ __device__ inline void snake_range(const Grid& g, int row, int x0, int x1, int& first, int& last) {
+  const int base = g.nc[0] * row;
+  if (row & 1) { first = base + g.nc[0] - 1 - x1; last = base + g.nc[0] - 1 - x0; }
+  else { first = base + x0; last = base + x1; }
+}
+/* physical cell coordinates of a cell id */
+__host__ __device__ inline void snake_decode(const Grid& g, uint32_t cid, int& cx, int& cy, int& cz) {
+  const int row = (int)(cid / (uint32_t)g.nc[0]);
+  const int xs = (int)(cid % (uint32_t)g.nc[0]);
+  cz = row / g.nc[1];
+  const int ys = row - cz * g.nc[1];
+  cy = (cz & 1) ? g.nc[1] - 1 - ys : ys;
+  cx = (row & 1) ? g.nc[0] - 1 - xs : xs;
+}
 
 /* geometry of a time slice: g = diag(1, -1, -1, -G3), G3 = tau^2 (hyperbolic) or 1 */
 struct Geom {
@@ -80,7 +104,7 @@ struct Sorted {
   /* pack: exact positions (SoA), FP32 positions relative to grid.xmin, AoS payload of the smoothing pass */
   double* x[3];
   float4* xf;
-  double* rec_s;      /* [n][8]: x[3], S, N_B, N_S, N_Q, m */
+  double* rec_s;      /* [n][8]: x[3], m, S, N_B, N_S, N_Q */
   /* a4 */
   double *sigma_star, *s_star, *rho_star[NQ];
   uint32_t* nnb;

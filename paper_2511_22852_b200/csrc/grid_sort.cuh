@@ -117,22 +117,41 @@ __device__ inline int cell_coord(double x, double xmin, double inv_edge, int nc)
   return c;
 }
 
-/* spread the low bits of v so that bit k lands at position k * stride */
-__device__ inline uint32_t spread_bits(uint32_t v, int nbits, int stride) {
-  uint32_t r = 0;
-  for (int k = 0; k < nbits; ++k) r |= ((v >> k) & 1u) << (k * stride);
-  return r;
+/* Hilbert index of the sub-cell (X[0..D-1], nb bits each): Skilling's transpose algorithm ("Programming the
+   Hilbert curve", 2004) followed by the bit interleave.  The curve visits every sub-cell once, consecutive
+   indices are face neighbours, and it runs from corner (0,..,0) to corner (max,0,..,0) — so with cells ordered x
+   fastest it continues into the next cell of the row without a jump.  Any bijection would be correct here;
+   this one makes every run of consecutive sorted particles spatially compact, which is what the pair kernels'
+   register tile (2 particles per thread, 2 threads per stream) needs. */
+__device__ inline uint32_t hilbert_index(uint32_t* X, int nb, int D) {
+  const uint32_t M = 1u << (nb - 1);
+  for (uint32_t Q = M; Q > 1u; Q >>= 1) {
+    const uint32_t P = Q - 1u;
+    for (int i = 0; i < D; ++i) {
+      if (X[i] & Q) X[0] ^= P;
+      else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+    }
+  }
+  for (int i = 1; i < D; ++i) X[i] ^= X[i - 1];
+  uint32_t t = 0;
+  for (uint32_t Q = M; Q > 1u; Q >>= 1)
+    if (X[D - 1] & Q) t ^= Q - 1u;
+  for (int i = 0; i < D; ++i) X[i] ^= t;
+  uint32_t h = 0;
+  for (int q = nb - 1; q >= 0; --q)
+    for (int i = 0; i < D; ++i) h = (h << 1) | ((X[i] >> q) & 1u);
+  return h;
 }
 
-/* sort key: traversal cell (x fastest) in the high bits; below it the Morton code of the position inside the
-   cell (3 bits per axis in 3-D, 4 in 2-D), so that consecutive particles of a cell form compact clusters */
+/* sort key: traversal cell (x fastest) in the high bits; below it the Hilbert index of the position inside the
+   cell (3 bits per axis in 3-D, 4 in 2-D), so that consecutive particles form compact clusters */
 __global__ void cell_hash_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
                                  const Grid* __restrict__ grid, uint32_t* __restrict__ key, uint32_t* __restrict__ val) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const Grid g = *grid;
   int c[3] = {0, 0, 0};
-  uint32_t morton = 0;
+  uint32_t sub3[3] = {0, 0, 0};
   const int sb = g.mb / D;               /* bits per axis */
   for (int k = 0; k < 3; ++k)
     if (k < D) {
@@ -140,10 +159,14 @@ __global__ void cell_hash_kernel(const double* __restrict__ Y, int64_t npad, int
       c[k] = cell_coord(x, g.xmin[k], g.inv_edge, g.nc[k]);
       const double frac = (x - g.xmin[k]) * g.inv_edge - (double)c[k];
       int sub = (int)(frac * (double)(1 << sb));
-      sub = max(0, min(sub, (1 << sb) - 1));
-      morton |= spread_bits((uint32_t)sub, sb, D) << k;
+      sub3[k] = (uint32_t)max(0, min(sub, (1 << sb) - 1));
     }
-  const uint32_t cell = (uint32_t)(c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2]));
+  const int row = snake_row(g, c[1], c[2]);
+  if (row & 1) sub3[0] = (uint32_t)((1 << sb) - 1) - sub3[0];      /* odd rows run backwards in x */
+  const uint32_t morton = hilbert_index(sub3, sb, D);
+  int cell_i, cell_last;
+  snake_range(g, row, c[0], c[0], cell_i, cell_last);
+  const uint32_t cell = (uint32_t)cell_i;
   key[i] = (cell << g.mb) | morton;
   val[i] = (uint32_t)i;
 }
@@ -319,7 +342,7 @@ __global__ void iota_kernel(uint32_t* __restrict__ p, int64_t n) {
 }
 
 /* sorted order: exact positions, FP32 positions relative to the grid origin (culling only), and the AoS payload
-   record of the smoothing pass: x[3], S, N_B, N_S, N_Q, m */
+   record of the smoothing pass: x[3], m, S, N_B, N_S, N_Q */
 __global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D,
                                       const uint32_t* __restrict__ perm, const Grid* __restrict__ grid, Sorted so) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -330,9 +353,9 @@ __global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad
   so.xf[i] = make_float4((float)(x - grid->xmin[0]), (float)(y - grid->xmin[1]), (D == 3) ? (float)(z - grid->xmin[2]) : 0.f, 0.f);
   double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
   r[0] = make_double2(x, y);
-  r[1] = make_double2(z, Y[CCAKE_S * npad + a]);
-  r[2] = make_double2(Y[CCAKE_NB * npad + a], Y[CCAKE_NS * npad + a]);
-  r[3] = make_double2(Y[CCAKE_NQ * npad + a], Y[CCAKE_MASS * npad + a]);
+  r[1] = make_double2(z, Y[CCAKE_MASS * npad + a]);
+  r[2] = make_double2(Y[CCAKE_S * npad + a], Y[CCAKE_NB * npad + a]);
+  r[3] = make_double2(Y[CCAKE_NS * npad + a], Y[CCAKE_NQ * npad + a]);
 }
 
 }  // namespace ccake
