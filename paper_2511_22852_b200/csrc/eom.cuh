@@ -44,7 +44,7 @@ struct EomOut {
 };
 
 template <int D>
-__device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
+__device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
                                        EomOut& o) {
   const double gam = in.gam, sig = in.sig;
   const double tau = gm.tau;
@@ -53,6 +53,7 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
   /* Eq. 97, nu = 0: u_0 du^0 = -u_k du^k - (1/2) u^a u^b dg_ab/dx0,  dg_33/dx0 = -dG3 */
   const double gt = -in.u[3] * in.u[3] * gm.dG3;
   du[0] = -(in.ulo[1] * du[1] + in.ulo[2] * du[2] + in.ulo[3] * du[3]) / gam - gt / (2.0 * gam);
+#pragma unroll
   for (int m = 0; m < 4; ++m) dulo[m] = in.glo[m] * du[m];
   dulo[3] += -gm.dG3 * in.u[3];
   o.du0 = du[0];
@@ -60,14 +61,20 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
   o.theta = theta;
   /* covariant derivative, acceleration */
   double CD[4][4], Du[4], Dulo[4];
-  for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) CD[m][n] = in.CDc[m][n];
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = 0; n < 4; ++n) CD[m][n] = in.CDc[m][n];
+#pragma unroll
   for (int n = 0; n < 4; ++n) { CD[0][n] += du[n]; Du[n] = in.Duc[n] + gam * du[n]; Dulo[n] = in.glo[n] * Du[n]; }
 
   const double Pi = in.ds.bulkt * sig;
   const bool need_sg = kp.shear || (kp.bulk && in.lambda_Pipi != 0.0);
   double sg[4][4];
   if (need_sg) {
+#pragma unroll
     for (int m = 0; m < 4; ++m)
+#pragma unroll
       for (int n = m; n < 4; ++n) {
         const double Delta = ((m == n) ? in.gup[m] : 0.0) - in.u[m] * in.u[n];
         const double v = 0.5 * (in.gup[m] * CD[m][n] + in.gup[n] * CD[n][m]) - 0.5 * (in.u[m] * Du[n] + in.u[n] * Du[m]) -
@@ -81,26 +88,37 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
     double rhs = -Pi - in.zeta * theta + (in.tau_Pi - in.delta_PiPi) * Pi * theta;
     if (in.lambda_Pipi != 0.0) {
       double acc = 0.0;
+#pragma unroll
       for (int m = 0; m < 4; ++m)
+#pragma unroll
         for (int n = 0; n < 4; ++n) acc += sig * in.ds.pit[m][n] * in.glo[m] * in.glo[n] * sg[m][n];
       rhs += in.lambda_Pipi * acc;
     }
     o.dBulk = rhs / (in.tau_Pi * sig * gam);
   }
   /* shear */
-  for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) o.dpit[m][n] = 0.0;
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = 0; n < 4; ++n) o.dpit[m][n] = 0.0;
   if (kp.shear) {
     double om[4][4];
     const bool need_om = in.phi_omega != 0.0;
     if (need_om)
+#pragma unroll
       for (int m = 0; m < 4; ++m)
+#pragma unroll
         for (int n = 0; n < 4; ++n)
           om[m][n] = 0.5 * (in.gup[m] * CD[m][n] - in.gup[n] * CD[n][m]) - 0.5 * (in.u[m] * Du[n] - in.u[n] * Du[m]);
     double Xtr = 0.0;
     if (in.tau_pipi != 0.0)
+#pragma unroll
       for (int l = 0; l < 4; ++l)
+#pragma unroll
         for (int m = 0; m < 4; ++m) Xtr += sig * in.ds.pit[l][m] * in.glo[l] * in.glo[m] * sg[m][l];
+#pragma unroll
     for (int i = 1; i <= 3; ++i)
+#pragma unroll
       for (int j = i; j <= 3; ++j) {
         if (D == 2 && j == 3 && i != 3) continue;          /* pi^{13}, pi^{23} vanish by symmetry in 2+1D */
         double conn = 0.0;                                  /* u^l Gamma^i_{l r} pi~^{r j} + (i <-> j)      */
@@ -109,11 +127,13 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
           if (j == 3) conn += (gam * in.ds.pit[i][3] + in.u[3] * in.ds.pit[i][0]) / tau;
         }
         double acc = 0.0;
+#pragma unroll
         for (int l = 0; l < 4; ++l) acc += (in.u[i] * in.ds.pit[j][l] + in.u[j] * in.ds.pit[i][l]) * Dulo[l];
         const double piij = sig * in.ds.pit[i][j];
         double rhs = -piij + 2.0 * in.eta * sg[i][j] + (in.tau_pi - in.delta_pipi) * piij * theta;
         if (in.tau_pipi != 0.0) {
           double X = 0.0;
+#pragma unroll
           for (int l = 0; l < 4; ++l) {
             X += 0.5 * sig * in.ds.pit[l][i] * in.glo[l] * sg[l][j];
             X += 0.5 * sig * in.ds.pit[l][j] * in.glo[l] * sg[l][i];
@@ -125,6 +145,7 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
         if (in.lambda_piPi != 0.0) rhs += in.lambda_piPi * Pi * sg[i][j];
         if (need_om) {
           double Yv = 0.0;
+#pragma unroll
           for (int l = 0; l < 4; ++l) {
             Yv += 0.5 * sig * in.ds.pit[i][l] * in.glo[l] * om[j][l];
             Yv += 0.5 * sig * in.ds.pit[j][l] * in.glo[l] * om[i][l];
@@ -135,44 +156,61 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
         o.dpit[i][j] = d; o.dpit[j][i] = d;
       }
     /* d/dx0 of u_mu pi~^{mu nu} = 0 */
+#pragma unroll
     for (int n = 1; n <= 3; ++n) {
       double acc = 0.0;
+#pragma unroll
       for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][n];
+#pragma unroll
       for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][n];
       o.dpit[0][n] = acc / gam; o.dpit[n][0] = acc / gam;
     }
     double acc = 0.0;
+#pragma unroll
     for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][0];
+#pragma unroll
     for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][0];
     o.dpit[0][0] = acc / gam;
   }
   /* diffusion */
-  for (int q = 0; q < NQ; ++q) for (int m = 0; m < 4; ++m) o.dJt[q][m] = 0.0;
+#pragma unroll
+  for (int q = 0; q < NQ; ++q)
+#pragma unroll
+    for (int m = 0; m < 4; ++m) o.dJt[q][m] = 0.0;
   if (kp.diff) {
+#pragma unroll
     for (int q = 0; q < NQ; ++q) {
       double JDu = 0.0;
+#pragma unroll
       for (int n = 0; n < 4; ++n) JDu += in.ds.Jt[q][n] * Dulo[n];
+#pragma unroll
       for (int i = 1; i <= D; ++i) {
         double conn = 0.0;
         if (gm.hyper && i == 3) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) / tau;
         o.dJt[q][i] = (in.rhsJ[q][i - 1] / (in.tau_q[q] * sig) - conn - in.u[i] * JDu) / gam;
       }
       double acc = 0.0;
+#pragma unroll
       for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.Jt[q][m];
+#pragma unroll
       for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dJt[q][j];
       o.dJt[q][0] = acc / gam;
     }
   }
   /* charge: d/dx0 [ N_q + J~^0_q / gamma ] = -sqrt(-g) FK_q */
+#pragma unroll
   for (int q = 0; q < NQ; ++q)
     o.dN[q] = -in.FKs[q] - o.dJt[q][0] / gam + (in.ds.Jt[q][0] / (gam * gam)) * du[0];
   /* entropy, Eq. 96: gamma sigma (T dS + mu_q dN_q) = -Pi theta + pi^mu_nu nabla_mu u^nu */
   {
     double rhs = -Pi * theta;
     if (kp.shear)
+#pragma unroll
       for (int m = 0; m < 4; ++m)
+#pragma unroll
         for (int n = 0; n < 4; ++n) rhs += sig * in.ds.pit[m][n] * in.glo[n] * CD[m][n];
     double lhs = 0.0;
+#pragma unroll
     for (int q = 0; q < NQ; ++q) lhs += gam * sig * in.mu[q] * o.dN[q];
     o.dS = (rhs - lhs) / (gam * sig * in.T);
   }
@@ -181,7 +219,9 @@ __device__ __noinline__ void eom_rates(const KParams& kp, const Geom& gm, const 
   const double A = w * in.cs2;
   const double Cc = w / sig + in.ds.bulkt;
   double dC = in.ws * o.dS + o.dBulk - (A / sig) * (theta / gam);
+#pragma unroll
   for (int q = 0; q < NQ; ++q) dC += in.wq[q] * o.dN[q];
+#pragma unroll
   for (int i = 1; i <= D; ++i) {
     const double pit0_lo = in.glo[i] * in.ds.pit[0][i];
     double dpit0_lo = in.glo[i] * o.dpit[0][i];
@@ -205,8 +245,11 @@ struct RkArgs {
   int update;           /* 0: rates only (refresh)                 */
 };
 
+#ifndef CCAKE_EOM_MINB
+#define CCAKE_EOM_MINB 2
+#endif
 template <int D>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, CCAKE_EOM_MINB)
 eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, uint32_t field_mask,
            Status* __restrict__ status) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -217,10 +260,12 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   load_u(kp, gm, Y, npad, a, in.u);
   in.gam = in.u[0];
   in.glo[0] = 1.0; in.glo[1] = -1.0; in.glo[2] = -1.0; in.glo[3] = -gm.G3;
+#pragma unroll
   for (int m = 0; m < 4; ++m) { in.gup[m] = 1.0 / in.glo[m]; in.ulo[m] = in.glo[m] * in.u[m]; in.v[m] = in.u[m] / in.gam; }
-  load_dissip(kp, gm, Y, npad, a, in.u, in.ds);
+  load_dissip<D>(kp, gm, Y, npad, a, in.u, in.ds);
   in.sig = so.sigma[i]; in.sst = so.sigma_star[i]; in.s = so.s[i];
   in.T = so.T[i]; in.p = so.p[i]; in.e = so.e[i]; in.cs2 = so.cs2[i]; in.ws = so.ws[i];
+#pragma unroll
   for (int q = 0; q < NQ; ++q) { in.mu[q] = so.mu[q][i]; in.wq[q] = kp.diff || kp.eos_kind == 0 ? so.wq[q][i] : so.wq[q][i]; }
   /* transport coefficients, §5.3 (:732-769), DESIGN reading 11 */
   {
@@ -232,7 +277,9 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
                   ? kp.zeta_max * (kp.zeta_width * kp.zeta_width) / (kp.zeta_width * kp.zeta_width + dT * dT) * in.s
                   : kp.zeta_max * in.s;
     in.tau_Pi = kp.tau_Pi_coeff * in.tau_pi;
+#pragma unroll
     for (int q = 0; q < NQ; ++q) {
+#pragma unroll
       for (int r = 0; r < NQ; ++r) in.kappa[q][r] = kp.kappa_over_T2[q * 3 + r] * in.T * in.T;
       in.tau_q[q] = kp.tau_q_times_T[q] / in.T;
     }
@@ -247,10 +294,15 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   /* gradients: d_k u^j from the SPH sums, d_k u^0 from u_mu d_k u^mu = 0, d_0 = d/dx0 - v^k d_k */
   {
     double PU[4][4];
-    for (int m = 0; m < 4; ++m) for (int nn = 0; nn < 4; ++nn) PU[m][nn] = 0.0;
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int nn = 0; nn < 4; ++nn) PU[m][nn] = 0.0;
     const double G[4] = {0.0, 1.0, 1.0, gm.G3};
+#pragma unroll
     for (int k = 1; k <= D; ++k) {
       double s0 = 0.0;
+#pragma unroll
       for (int j = 1; j <= D; ++j) {
         const double d = so.DU[(k - 1) * 3 + (j - 1)][i];
         PU[k][j] = d;
@@ -258,37 +310,51 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       }
       PU[k][0] = s0 / in.gam;
     }
+#pragma unroll
     for (int nn = 0; nn < 4; ++nn) {
       double s0 = 0.0;
+#pragma unroll
       for (int k = 1; k <= 3; ++k) s0 -= in.v[k] * PU[k][nn];
       PU[0][nn] = s0;                                         /* + du^nn, added per trial */
     }
-    for (int m = 0; m < 4; ++m) for (int nn = 0; nn < 4; ++nn) in.CDc[m][nn] = PU[m][nn];
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int nn = 0; nn < 4; ++nn) in.CDc[m][nn] = PU[m][nn];
     if (gm.hyper) {
       in.CDc[3][0] += gm.tau * in.u[3];          /* Gamma^0_{33} u^3 */
       in.CDc[0][3] += in.u[3] / gm.tau;          /* Gamma^3_{03} u^3 */
       in.CDc[3][3] += in.gam / gm.tau;           /* Gamma^3_{30} u^0 */
     }
+#pragma unroll
     for (int nn = 0; nn < 4; ++nn) {
       double s0 = 0.0;
+#pragma unroll
       for (int m = 0; m < 4; ++m) s0 += in.u[m] * in.CDc[m][nn];
       in.Duc[nn] = s0;
     }
   }
   in.thc = in.gam * (so.divv[i] + gm.Gamma_g);
+#pragma unroll
   for (int k = 0; k < 3; ++k) in.FM[k] = (k < D) ? gm.sqrtg * (so.FP[k][i] - so.FB[k][i]) : 0.0;
+#pragma unroll
   for (int q = 0; q < NQ; ++q) in.FKs[q] = gm.sqrtg * so.FK[q][i];
   if (kp.diff) {
     /* tau_q sigma [...] = -J^i_q + sum_q' kappa_qq' nabla^<i> alpha_q',  nabla^<i> alpha = g^{ii} d_i alpha - u^i u^j d_j alpha */
     double udota[NQ];
+#pragma unroll
     for (int r = 0; r < NQ; ++r) {
       double s0 = 0.0;
+#pragma unroll
       for (int j = 1; j <= D; ++j) s0 += in.u[j] * so.DA[r * 3 + (j - 1)][i];
       udota[r] = s0;
     }
+#pragma unroll
     for (int q = 0; q < NQ; ++q)
+#pragma unroll
       for (int k = 1; k <= D; ++k) {
         double rhs = -in.sig * in.ds.Jt[q][k];
+#pragma unroll
         for (int r = 0; r < NQ; ++r) rhs += in.kappa[q][r] * (in.gup[k] * so.DA[r * 3 + (k - 1)][i] - in.u[k] * udota[r]);
         in.rhsJ[q][k - 1] = rhs;
       }
@@ -298,35 +364,45 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   EomOut o;
   double r0[3], M[3][3], du[3] = {0.0, 0.0, 0.0};
   eom_rates<D>(kp, gm, in, du, o);
+#pragma unroll
   for (int k = 0; k < D; ++k) r0[k] = o.res[k];
-#pragma unroll 1
+#pragma unroll
   for (int c = 0; c < D; ++c) {
     double e[3] = {0.0, 0.0, 0.0};
     e[c] = 1.0;
     eom_rates<D>(kp, gm, in, e, o);
+#pragma unroll
     for (int k = 0; k < D; ++k) M[k][c] = o.res[k] - r0[k];
   }
   /* Gaussian elimination with partial pivoting */
   double b[3];
   bool ok = true;
+#pragma unroll
   for (int k = 0; k < D; ++k) b[k] = -r0[k];
+#pragma unroll
   for (int c = 0; c < D; ++c) {
     int piv = c;
+#pragma unroll
     for (int r = c + 1; r < D; ++r) if (fabs(M[r][c]) > fabs(M[piv][c])) piv = r;
     if (M[piv][c] == 0.0 || !(fabs(M[piv][c]) < INFINITY)) { ok = false; break; }
     if (piv != c) {
+#pragma unroll
       for (int k = 0; k < D; ++k) { const double t = M[c][k]; M[c][k] = M[piv][k]; M[piv][k] = t; }
       const double t = b[c]; b[c] = b[piv]; b[piv] = t;
     }
+#pragma unroll
     for (int r = c + 1; r < D; ++r) {
       const double f = M[r][c] / M[c][c];
+#pragma unroll
       for (int k = c; k < D; ++k) M[r][k] -= f * M[c][k];
       b[r] -= f * b[c];
     }
   }
   if (ok)
+#pragma unroll
     for (int r = D - 1; r >= 0; --r) {
       double s0 = b[r];
+#pragma unroll
       for (int k = r + 1; k < D; ++k) s0 -= M[r][k] * du[k];
       du[r] = s0 / M[r][r];
     }
@@ -335,14 +411,20 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
 
   /* rates of the evolved set */
   double k_[NSTATE];
+#pragma unroll
   for (int f = 0; f < NSTATE; ++f) k_[f] = 0.0;
+#pragma unroll
   for (int j = 1; j <= D; ++j) { k_[CCAKE_R1 + j - 1] = in.u[j] / in.gam; k_[CCAKE_U1 + j - 1] = du[j - 1]; }
   k_[CCAKE_S] = o.dS;
+#pragma unroll
   for (int q = 0; q < NQ; ++q) k_[CCAKE_NB + q] = o.dN[q];
   k_[CCAKE_BULK] = o.dBulk;
   k_[CCAKE_PI11] = o.dpit[1][1]; k_[CCAKE_PI12] = o.dpit[1][2]; k_[CCAKE_PI22] = o.dpit[2][2]; k_[CCAKE_PI33] = o.dpit[3][3];
   if (D == 3) { k_[CCAKE_PI13] = o.dpit[1][3]; k_[CCAKE_PI23] = o.dpit[2][3]; }
-  for (int q = 0; q < NQ; ++q) for (int j = 1; j <= D; ++j) k_[CCAKE_JB1 + 3 * q + j - 1] = o.dJt[q][j];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q)
+#pragma unroll
+    for (int j = 1; j <= D; ++j) k_[CCAKE_JB1 + 3 * q + j - 1] = o.dJt[q][j];
   /* 2+1D hyperbolic: longitudinal work rate (DESIGN reading 14) */
   if (gm.hyper && D == 2) {
     const double Pi = in.ds.bulkt * in.sig;
@@ -350,8 +432,10 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   }
   if (rk.theta_out) rk.theta_out[i] = o.theta;
   if (rk.Krate)
+#pragma unroll
     for (int f = 0; f < NSTATE; ++f) if (f != CCAKE_MASS) rk.Krate[f * npad + a] = k_[f];
   if (rk.update) {
+#pragma unroll
     for (int f = 0; f < NSTATE; ++f) {
       if (!(field_mask & (1u << f)) || f == CCAKE_MASS) continue;
       const double y0 = rk.Ybase[f * npad + a];

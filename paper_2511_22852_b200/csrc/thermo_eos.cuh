@@ -145,12 +145,14 @@ __device__ inline ThermoOut eos_closed_form(const KParams& kp, double s, const d
    u_mu pi^{mu nu} = 0 and u_mu J^mu = 0 (never evolved; DESIGN reading 13) */
 struct Dissip { double pit[4][4], Jt[NQ][4], bulkt; };
 
-__device__ inline void load_dissip(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad,
-                                   int64_t a, const double u[4], Dissip& ds) {
-  const int D = kp.D;
+template <int D>
+__device__ __forceinline__ void load_dissip(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad,
+                                            int64_t a, const double u[4], Dissip& ds) {
   const double gam = u[0];
   const double G[4] = {0.0, 1.0, 1.0, gm.G3};
+#pragma unroll
   for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) ds.pit[m][n] = 0.0;
+#pragma unroll
   for (int q = 0; q < NQ; ++q) for (int m = 0; m < 4; ++m) ds.Jt[q][m] = 0.0;
   ds.bulkt = kp.bulk ? Y[CCAKE_BULK * npad + a] : 0.0;
   if (kp.shear) {
@@ -162,19 +164,25 @@ __device__ inline void load_dissip(const KParams& kp, const Geom& gm, const doub
       ds.pit[1][3] = ds.pit[3][1] = Y[CCAKE_PI13 * npad + a];
       ds.pit[2][3] = ds.pit[3][2] = Y[CCAKE_PI23 * npad + a];
     }
+#pragma unroll
     for (int i = 1; i <= 3; ++i) {
       double acc = 0.0;
+#pragma unroll
       for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.pit[j][i];
       ds.pit[0][i] = ds.pit[i][0] = acc / gam;
     }
     double acc = 0.0;
+#pragma unroll
     for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.pit[j][0];
     ds.pit[0][0] = acc / gam;
   }
   if (kp.diff) {
+#pragma unroll
     for (int q = 0; q < NQ; ++q) {
+#pragma unroll
       for (int i = 1; i <= D; ++i) ds.Jt[q][i] = Y[(CCAKE_JB1 + 3 * q + (i - 1)) * npad + a];
       double acc = 0.0;
+#pragma unroll
       for (int j = 1; j <= 3; ++j) acc += G[j] * u[j] * ds.Jt[q][j];
       ds.Jt[q][0] = acc / gam;
     }
@@ -212,7 +220,8 @@ thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restr
     so.n[q][i] = nq[q]; so.mu[q][i] = th.mu[q]; so.wq[q][i] = th.wq[q];
   }
   Dissip ds;
-  load_dissip(kp, gm, Y, npad, a, u, ds);
+  if (D == 3) load_dissip<3>(kp, gm, Y, npad, a, u, ds);
+  else load_dissip<2>(kp, gm, Y, npad, a, u, ds);
   const double sst2 = sst * sst;
   const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
   /* AoS payload record of the gradient pass (layout GLayout): x[D], m, P, u[D], v[D], B[D*D], K[3*D], alpha[3] */

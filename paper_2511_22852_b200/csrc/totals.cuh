@@ -26,7 +26,8 @@ totals_partial_kernel(int64_t n, KParams kp, Geom gm, const double* __restrict__
     load_u(kp, gm, Y, npad, a, u);
     const double gam = u[0], sig = so.sigma[i], m = Y[CCAKE_MASS * npad + a];
     Dissip ds;
-    load_dissip(kp, gm, Y, npad, a, u, ds);
+    if (D == 3) load_dissip<3>(kp, gm, Y, npad, a, u, ds);
+    else load_dissip<2>(kp, gm, Y, npad, a, u, ds);
     const double p = so.p[i], w = so.e[i] + p, Pi = ds.bulkt * sig;
     const double Cc = (w + Pi) / sig;
     const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
