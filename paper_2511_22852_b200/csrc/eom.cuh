@@ -362,17 +362,22 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
 
   /* residual at du = 0 and at the unit vectors -> D x D system of Eq. 95 */
   EomOut o;
-  double r0[3], M[3][3], du[3] = {0.0, 0.0, 0.0};
+  double r0[3], M[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}}, du[3] = {0.0, 0.0, 0.0};
   eom_rates<D>(kp, gm, in, du, o);
 #pragma unroll
   for (int k = 0; k < D; ++k) r0[k] = o.res[k];
-#pragma unroll
+  /* one copy of the rate evaluation for all D columns (the instruction cache matters: the evaluation is a few
+     thousand instructions); unit vector and column store by selects, so no array is indexed dynamically */
+#pragma unroll 1
   for (int c = 0; c < D; ++c) {
-    double e[3] = {0.0, 0.0, 0.0};
-    e[c] = 1.0;
+    const double e[3] = {c == 0 ? 1.0 : 0.0, c == 1 ? 1.0 : 0.0, c == 2 ? 1.0 : 0.0};
     eom_rates<D>(kp, gm, in, e, o);
 #pragma unroll
-    for (int k = 0; k < D; ++k) M[k][c] = o.res[k] - r0[k];
+    for (int k = 0; k < D; ++k) {
+      const double m = o.res[k] - r0[k];
+#pragma unroll
+      for (int cc = 0; cc < D; ++cc) M[k][cc] = (cc == c) ? m : M[k][cc];
+    }
   }
   /* Gaussian elimination with partial pivoting */
   double b[3];
