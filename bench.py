@@ -49,6 +49,10 @@ def flop_grad_per_pair(D, visc, diff):
 
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+# capture of this command (profiles/r1f_README.md); only valid for the workload it was taken on
+NCU_TRAFFIC_BYTES = {("C4", "grad"): 1.612528e9 + 0.424980e9, ("C4", "smooth"): 0.289711e9 + 0.074932e9}
+
 
 def make_workload(name, rank=0, tiles=None):
     from paper_2511_22852_b200 import workloads as W
@@ -319,7 +323,9 @@ def run_ours(args):
             "substep_hbm_frac": total_bytes * nsub / (ms_total / args.steps * 1e-3) / 1e9 / hbm,
             "roofline": {"bound": "alu", "kernel": {"grad": "gradient pass a6", "smooth": "smoothing pass a4"}[dom],
                          "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
-                         "traffic": None, "peak_source": "fp64 DFMA: 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)) if args.tiles is None else None,
+                         "traffic_unit": "bytes per launch (ncu --set full, profiles/r1f_README.md)",
+                         "algorithmic_bytes": bytes_pp[dom] * w.n, "peak_source": "fp64 DFMA: 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md)",
                          "flop_per_pair": fg if dom == "grad" else FLOP_SMOOTH_PER_PAIR,
                          "hbm_peak_GBps": hbm, "hbm_peak_source": which},
             "kernels": kernels,
