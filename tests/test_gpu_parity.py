@@ -182,3 +182,52 @@ def test_runs_are_reproducible():
     for k in res[0][0]:
         assert np.array_equal(res[0][0][k], res[1][0][k])
     assert np.array_equal(res[0][1], res[1][1])
+
+
+def test_full_size_c4_sampled_event_tile():
+    """BASELINE.json configs[3] at full size (1,984,000 particles, the launch configuration bench.py times), checked
+    on a sample the oracle can afford: the event tiles are independent (gaps > 2h + twice the run's reach), so the
+    oracle run on the particles of ONE tile — the very same coordinates and fields, sliced out of the full input —
+    gives the exact expectation for those particles.  Neighbour counts bit-exact, smoothed densities 1e-11 element
+    by element, thermodynamics 1e-11, gradient sums 1e-10, and every evolved field 1e-8 after one RK2 step."""
+    tb = W.make_eos_table(100, 32, with_wq=True)
+    w = W.config_c4(table=tb)
+    K = w.meta["tiles"]
+    nt = w.n // K
+    t = 7
+    sl = slice(t * nt, (t + 1) * nt)
+    g = B.from_workload(w)
+    o = O.Oracle(**w.params)
+    o.load_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"], tb["data"])
+    o.load_particles({k: np.ascontiguousarray(v[sl]) for k, v in w.fields.items()})
+
+    def compare(ids, tol, what, elementwise=()):
+        fg, fo = g.read_fields(ids), o.read_fields(ids)
+        bad = {}
+        for k in ids:
+            a, b = fg[k][sl], fo[k]
+            assert np.all(np.isfinite(a)), (what, k)
+            if k in elementwise:
+                with np.errstate(divide="ignore", invalid="ignore"):
+                    r = np.abs(a - b) / np.abs(b)
+                r[a == b] = 0.0
+                e = float(r.max())
+            else:
+                e = norm_rel(a, b)
+            if not e <= tol:
+                bad[k] = e
+        assert not bad, f"{what}: beyond {tol:g}: {bad}"
+
+    ng = g.read_fields([B.NNB])[B.NNB][sl]
+    no = o.read_fields([O.NNB])[O.NNB]
+    assert np.array_equal(ng, no), "neighbour counts differ on the sampled tile"
+    sums = [B.SIGMA_STAR, B.S_STAR, B.RHOSTAR_B, B.RHOSTAR_S, B.RHOSTAR_Q]
+    compare(sums, TOL_SUM, "smoothing sums", elementwise=sums)
+    compare([B.T, B.P, B.E, B.MU_B, B.MU_S, B.MU_Q], TOL_SUM, "thermodynamics")
+    compare(gradient_ids(w.params), TOL_GRAD, "gradient sums")
+    g.step(1)
+    g.synchronize()
+    o.step(1)
+    compare(state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, "fields after one RK2 step",
+            elementwise=(B.SIGMA_STAR, B.T, B.P))
+    g.close()
