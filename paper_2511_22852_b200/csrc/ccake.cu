@@ -50,6 +50,8 @@ struct ccake_ctx {
   double *tot_partial = nullptr, *tot_out = nullptr;
   int tot_blocks = 0;
   double* arena = nullptr;      /* sorted-order doubles */
+  ulonglong2* mask_cache = nullptr;   /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
+  int mask_tiles = 0;
   uint32_t* nnb = nullptr;
   double* theta = nullptr;
   double* scratch = nullptr;    /* N doubles: read_fields staging */
@@ -97,6 +99,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->tot_partial); c->tot_partial = nullptr;
   cudaFree(c->tot_out); c->tot_out = nullptr;
   cudaFree(c->arena); c->arena = nullptr;
+  cudaFree(c->mask_cache); c->mask_cache = nullptr; c->mask_tiles = 0;
   cudaFree(c->nnb); c->nnb = nullptr;
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
@@ -148,6 +151,8 @@ void carve(ccake_ctx* c) {
   s.divv = take();
   s.nnb = c->nnb;
   s.cell_start = c->cell_start;
+  s.mask_cache = c->mask_cache;
+  s.mask_tiles = c->mask_tiles;
 }
 
 int launch_check(ccake_ctx* c, const char* what) {
@@ -519,6 +524,17 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   }
   CK(cudaMalloc(&c->arena, sizeof(double) * np * ARENA_FIELDS));
   CK(cudaMemsetAsync(c->arena, 0, sizeof(double) * np * ARENA_FIELDS, c->stream));
+  {
+    /* hit-mask cache: MASK_TILES tiles per pair block, 16 B per stream and tile; capped at 1/8 of the free memory
+       and dropped altogether if the allocation fails — the gradient pass then computes its masks itself */
+    const size_t nblocks = (size_t)((c->N + BH - 1) / BH), per_tile = sizeof(ulonglong2) * (PT / CCAKE_PAIR_LPS);
+    size_t free_b = 0, total_b = 0;
+    int tiles = MASK_TILES;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess)
+      while (tiles > 0 && nblocks * tiles * per_tile > free_b / 8) tiles /= 2;
+    if (tiles > 0 && cudaMalloc(&c->mask_cache, nblocks * tiles * per_tile) == cudaSuccess) c->mask_tiles = tiles;
+    else { cudaGetLastError(); c->mask_cache = nullptr; c->mask_tiles = 0; }
+  }
   CK(cudaMalloc(&c->nnb, sizeof(uint32_t) * np));
   CK(cudaMalloc(&c->theta, sizeof(double) * np));
   CK(cudaMalloc(&c->scratch, sizeof(double) * np));

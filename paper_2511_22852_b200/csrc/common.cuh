@@ -114,6 +114,10 @@ struct Sorted {
   double* rec_g;      /* [n][NREC]: AoS payload of the gradient pass, layout GLayout (pair_tiled.cuh) */
   /* a6 */
   double *FP[3], *FB[3], *FK[NQ], *DU[9], *DA[9], *divv;
+  /* hit masks of the smoothing pass, reused by the gradient pass of the same substep (pair_tiled.cuh):
+     [pair block][tile number < mask_tiles][stream] x 128 bit; NULL / 0 = no reuse */
+  ulonglong2* mask_cache;
+  int mask_tiles;
 };
 
 /* device-side status counters */
