@@ -433,6 +433,8 @@ int ccake_create(const ccake_params* p, ccake_ctx** out) {
   { const double twoh = 2.0 * p->h; k.cut2 = twoh * twoh; }
   const double pi = 3.14159265358979323846;
   k.sigma_d = (p->dim == 2) ? 10.0 / (7.0 * pi * p->h * p->h) : 1.0 / (pi * p->h * p->h * p->h);
+  k.w_a = 0.75 * k.sigma_d; k.w_b = -1.5 * k.sigma_d; k.w_c = 0.25 * k.sigma_d;
+  k.g_a = 2.25 * k.sigma_d / (p->h * p->h); k.g_b = -3.0 * k.sigma_d / (p->h * p->h); k.g_c = -0.75 * k.sigma_d / p->h;
   k.c0 = p->eos_c0; k.c2 = p->eos_c2; k.c4 = p->eos_c4;
   k.eta_over_s = p->eta_over_s; k.tau_pi_coeff = p->tau_pi_coeff; k.tau_floor = p->tau_floor;
   k.zeta_max = p->zeta_max; k.zeta_T_peak = p->zeta_T_peak; k.zeta_width = p->zeta_width; k.tau_Pi_coeff = p->tau_Pi_coeff;

@@ -82,6 +82,10 @@ struct KParams {
   int D, coords, eom, eos_kind;
   int shear, bulk, diff;
   double h, inv_h, cut2, sigma_d;   /* kernel normalisation sigma_D of Eq. 77 */
+  /* folded constants of the cubic spline (Eq. 77, 79), set once on the host so that the pair kernels read them as
+     constant-bank operands:  W = sigma_D (1 - 3/2 q^2 + 3/4 q^3) | sigma_D/4 (2-q)^3;
+     (grad W)/dr = sigma_D/h^2 (9/4 q - 3) | -3/4 sigma_D/h (2-q)^2 / r */
+  double w_a, w_b, w_c, g_a, g_b, g_c;
   double c0, c2, c4;
   double eta_over_s, tau_pi_coeff, tau_floor;
   double zeta_max, zeta_T_peak, zeta_width, tau_Pi_coeff;
