@@ -28,6 +28,9 @@ namespace ccake {
 struct EomIn {
   double u[4], ulo[4], v[4], glo[4], gup[4];
   double gam, sig, sst, T, mu[NQ], p, e, cs2, ws, wq[NQ], s;
+  /* reciprocals, taken once per particle (a double division is ~25 instructions; the rate evaluation runs D + 2
+     times): 1/gamma, 1/tau, 1/sigma, 1/(tau_Pi sigma gamma), 1/(sigma tau_pi), 1/(tau_q sigma), 1/(gamma sigma T) */
+  double igam, itau, isig, i_tauPi_sig_gam, i_sig_taupi, i_tauq_sig[NQ], i_gam_sig_T;
   double eta, zeta, tau_pi, tau_Pi, kappa[NQ][NQ], tau_q[NQ];
   double delta_PiPi, lambda_Pipi, delta_pipi, tau_pipi, lambda_piPi, phi_omega;
   double CDc[4][4];      /* nabla_mu u^nu without the du^nu part of the row mu = 0 */
@@ -47,12 +50,12 @@ template <int D>
 __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
                                        EomOut& o) {
   const double gam = in.gam, sig = in.sig;
-  const double tau = gm.tau;
+  const double igam = in.igam, itau = in.itau;
   double du[4], dulo[4];
   du[1] = du_in[0]; du[2] = du_in[1]; du[3] = (D == 3) ? du_in[2] : 0.0;
   /* Eq. 97, nu = 0: u_0 du^0 = -u_k du^k - (1/2) u^a u^b dg_ab/dx0,  dg_33/dx0 = -dG3 */
   const double gt = -in.u[3] * in.u[3] * gm.dG3;
-  du[0] = -(in.ulo[1] * du[1] + in.ulo[2] * du[2] + in.ulo[3] * du[3]) / gam - gt / (2.0 * gam);
+  du[0] = -(in.ulo[1] * du[1] + in.ulo[2] * du[2] + in.ulo[3] * du[3]) * igam - gt * (0.5 * igam);
 #pragma unroll
   for (int m = 0; m < 4; ++m) dulo[m] = in.glo[m] * du[m];
   dulo[3] += -gm.dG3 * in.u[3];
@@ -78,7 +81,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
       for (int n = m; n < 4; ++n) {
         const double Delta = ((m == n) ? in.gup[m] : 0.0) - in.u[m] * in.u[n];
         const double v = 0.5 * (in.gup[m] * CD[m][n] + in.gup[n] * CD[n][m]) - 0.5 * (in.u[m] * Du[n] + in.u[n] * Du[m]) -
-                         (Delta / 3.0) * theta;
+                         (Delta * (1.0 / 3.0)) * theta;
         sg[m][n] = v; sg[n][m] = v;
       }
   }
@@ -94,7 +97,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
         for (int n = 0; n < 4; ++n) acc += sig * in.ds.pit[m][n] * in.glo[m] * in.glo[n] * sg[m][n];
       rhs += in.lambda_Pipi * acc;
     }
-    o.dBulk = rhs / (in.tau_Pi * sig * gam);
+    o.dBulk = rhs * in.i_tauPi_sig_gam;
   }
   /* shear */
 #pragma unroll
@@ -123,8 +126,8 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
         if (D == 2 && j == 3 && i != 3) continue;          /* pi^{13}, pi^{23} vanish by symmetry in 2+1D */
         double conn = 0.0;                                  /* u^l Gamma^i_{l r} pi~^{r j} + (i <-> j)      */
         if (gm.hyper) {
-          if (i == 3) conn += (gam * in.ds.pit[3][j] + in.u[3] * in.ds.pit[0][j]) / tau;
-          if (j == 3) conn += (gam * in.ds.pit[i][3] + in.u[3] * in.ds.pit[i][0]) / tau;
+          if (i == 3) conn += (gam * in.ds.pit[3][j] + in.u[3] * in.ds.pit[0][j]) * itau;
+          if (j == 3) conn += (gam * in.ds.pit[i][3] + in.u[3] * in.ds.pit[i][0]) * itau;
         }
         double acc = 0.0;
 #pragma unroll
@@ -139,7 +142,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
             X += 0.5 * sig * in.ds.pit[l][j] * in.glo[l] * sg[l][i];
           }
           const double Delta = ((i == j) ? in.gup[i] : 0.0) - in.u[i] * in.u[j];
-          X -= (Delta / 3.0) * Xtr;
+          X -= (Delta * (1.0 / 3.0)) * Xtr;
           rhs -= in.tau_pipi * X;
         }
         if (in.lambda_piPi != 0.0) rhs += in.lambda_piPi * Pi * sg[i][j];
@@ -152,7 +155,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
           }
           rhs += 2.0 * in.tau_pi * in.phi_omega * Yv;
         }
-        const double d = (rhs / (sig * in.tau_pi) - conn - acc) / gam;
+        const double d = (rhs * in.i_sig_taupi - conn - acc) * igam;
         o.dpit[i][j] = d; o.dpit[j][i] = d;
       }
     /* d/dx0 of u_mu pi~^{mu nu} = 0 */
@@ -163,14 +166,14 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
       for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][n];
 #pragma unroll
       for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][n];
-      o.dpit[0][n] = acc / gam; o.dpit[n][0] = acc / gam;
+      o.dpit[0][n] = acc * igam; o.dpit[n][0] = acc * igam;
     }
     double acc = 0.0;
 #pragma unroll
     for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.pit[m][0];
 #pragma unroll
     for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dpit[j][0];
-    o.dpit[0][0] = acc / gam;
+    o.dpit[0][0] = acc * igam;
   }
   /* diffusion */
 #pragma unroll
@@ -186,21 +189,21 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
 #pragma unroll
       for (int i = 1; i <= D; ++i) {
         double conn = 0.0;
-        if (gm.hyper && i == 3) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) / tau;
-        o.dJt[q][i] = (in.rhsJ[q][i - 1] / (in.tau_q[q] * sig) - conn - in.u[i] * JDu) / gam;
+        if (gm.hyper && i == 3) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) * itau;
+        o.dJt[q][i] = (in.rhsJ[q][i - 1] * in.i_tauq_sig[q] - conn - in.u[i] * JDu) * igam;
       }
       double acc = 0.0;
 #pragma unroll
       for (int m = 0; m < 4; ++m) acc -= dulo[m] * in.ds.Jt[q][m];
 #pragma unroll
       for (int j = 1; j <= 3; ++j) acc -= in.ulo[j] * o.dJt[q][j];
-      o.dJt[q][0] = acc / gam;
+      o.dJt[q][0] = acc * igam;
     }
   }
   /* charge: d/dx0 [ N_q + J~^0_q / gamma ] = -sqrt(-g) FK_q */
 #pragma unroll
   for (int q = 0; q < NQ; ++q)
-    o.dN[q] = -in.FKs[q] - o.dJt[q][0] / gam + (in.ds.Jt[q][0] / (gam * gam)) * du[0];
+    o.dN[q] = -in.FKs[q] - o.dJt[q][0] * igam + (in.ds.Jt[q][0] * (igam * igam)) * du[0];
   /* entropy, Eq. 96: gamma sigma (T dS + mu_q dN_q) = -Pi theta + pi^mu_nu nabla_mu u^nu */
   {
     double rhs = -Pi * theta;
@@ -212,13 +215,13 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
     double lhs = 0.0;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) lhs += gam * sig * in.mu[q] * o.dN[q];
-    o.dS = (rhs - lhs) / (gam * sig * in.T);
+    o.dS = (rhs - lhs) * in.i_gam_sig_T;
   }
   /* momentum residual */
   const double w = in.e + in.p;
   const double A = w * in.cs2;
-  const double Cc = w / sig + in.ds.bulkt;
-  double dC = in.ws * o.dS + o.dBulk - (A / sig) * (theta / gam);
+  const double Cc = w * in.isig + in.ds.bulkt;
+  double dC = in.ws * o.dS + o.dBulk - (A * in.isig) * (theta * igam);
 #pragma unroll
   for (int q = 0; q < NQ; ++q) dC += in.wq[q] * o.dN[q];
 #pragma unroll
@@ -226,7 +229,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
     const double pit0_lo = in.glo[i] * in.ds.pit[0][i];
     double dpit0_lo = in.glo[i] * o.dpit[0][i];
     if (i == 3) dpit0_lo += -gm.dG3 * in.ds.pit[0][3];
-    o.res[i - 1] = in.ulo[i] * dC + Cc * dulo[i] + dpit0_lo / gam - (pit0_lo / (gam * gam)) * du[0] - in.FM[i - 1];
+    o.res[i - 1] = in.ulo[i] * dC + Cc * dulo[i] + dpit0_lo * igam - (pit0_lo * (igam * igam)) * du[0] - in.FM[i - 1];
   }
 }
 
@@ -290,6 +293,14 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       in.delta_pipi = kp.dnmr[2] * in.tau_pi; in.tau_pipi = kp.dnmr[3] * in.tau_pi;
       in.lambda_piPi = kp.dnmr[4]; in.phi_omega = kp.dnmr[5];
     }
+  in.igam = 1.0 / in.gam;
+  in.itau = 1.0 / gm.tau;
+  in.isig = 1.0 / in.sig;
+  in.i_tauPi_sig_gam = 1.0 / (in.tau_Pi * in.sig * in.gam);
+  in.i_sig_taupi = 1.0 / (in.sig * in.tau_pi);
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) in.i_tauq_sig[q] = 1.0 / (in.tau_q[q] * in.sig);
+  in.i_gam_sig_T = 1.0 / (in.gam * in.sig * in.T);
   }
   /* gradients: d_k u^j from the SPH sums, d_k u^0 from u_mu d_k u^mu = 0, d_0 = d/dx0 - v^k d_k */
   {
