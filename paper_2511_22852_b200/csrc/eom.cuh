@@ -262,9 +262,11 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   EomIn in;
   load_u(kp, gm, Y, npad, a, in.u);
   in.gam = in.u[0];
+  in.igam = 1.0 / in.gam;
+  in.itau = gm.hyper ? 1.0 / gm.tau : 0.0;
   in.glo[0] = 1.0; in.glo[1] = -1.0; in.glo[2] = -1.0; in.glo[3] = -gm.G3;
 #pragma unroll
-  for (int m = 0; m < 4; ++m) { in.gup[m] = 1.0 / in.glo[m]; in.ulo[m] = in.glo[m] * in.u[m]; in.v[m] = in.u[m] / in.gam; }
+  for (int m = 0; m < 4; ++m) { in.gup[m] = (m == 3) ? -1.0 / gm.G3 : in.glo[m]; in.ulo[m] = in.glo[m] * in.u[m]; in.v[m] = in.u[m] * in.igam; }
   load_dissip<D>(kp, gm, Y, npad, a, in.u, in.ds);
   in.sig = so.sigma[i]; in.sst = so.sigma_star[i]; in.s = so.s[i];
   in.T = so.T[i]; in.p = so.p[i]; in.e = so.e[i]; in.cs2 = so.cs2[i]; in.ws = so.ws[i];
@@ -293,8 +295,6 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       in.delta_pipi = kp.dnmr[2] * in.tau_pi; in.tau_pipi = kp.dnmr[3] * in.tau_pi;
       in.lambda_piPi = kp.dnmr[4]; in.phi_omega = kp.dnmr[5];
     }
-  in.igam = 1.0 / in.gam;
-  in.itau = 1.0 / gm.tau;
   in.isig = 1.0 / in.sig;
   in.i_tauPi_sig_gam = 1.0 / (in.tau_Pi * in.sig * in.gam);
   in.i_sig_taupi = 1.0 / (in.sig * in.tau_pi);
@@ -319,7 +319,7 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
         PU[k][j] = d;
         s0 += G[j] * in.u[j] * d;
       }
-      PU[k][0] = s0 / in.gam;
+      PU[k][0] = s0 * in.igam;
     }
 #pragma unroll
     for (int nn = 0; nn < 4; ++nn) {
@@ -334,8 +334,8 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       for (int nn = 0; nn < 4; ++nn) in.CDc[m][nn] = PU[m][nn];
     if (gm.hyper) {
       in.CDc[3][0] += gm.tau * in.u[3];          /* Gamma^0_{33} u^3 */
-      in.CDc[0][3] += in.u[3] / gm.tau;          /* Gamma^3_{03} u^3 */
-      in.CDc[3][3] += in.gam / gm.tau;           /* Gamma^3_{30} u^0 */
+      in.CDc[0][3] += in.u[3] * in.itau;          /* Gamma^3_{03} u^3 */
+      in.CDc[3][3] += in.gam * in.itau;           /* Gamma^3_{30} u^0 */
     }
 #pragma unroll
     for (int nn = 0; nn < 4; ++nn) {
@@ -430,7 +430,7 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
 #pragma unroll
   for (int f = 0; f < NSTATE; ++f) k_[f] = 0.0;
 #pragma unroll
-  for (int j = 1; j <= D; ++j) { k_[CCAKE_R1 + j - 1] = in.u[j] / in.gam; k_[CCAKE_U1 + j - 1] = du[j - 1]; }
+  for (int j = 1; j <= D; ++j) { k_[CCAKE_R1 + j - 1] = in.u[j] * in.igam; k_[CCAKE_U1 + j - 1] = du[j - 1]; }
   k_[CCAKE_S] = o.dS;
 #pragma unroll
   for (int q = 0; q < NQ; ++q) k_[CCAKE_NB + q] = o.dN[q];
