@@ -249,7 +249,7 @@ struct RkArgs {
 };
 
 #ifndef CCAKE_EOM_MINB
-#define CCAKE_EOM_MINB 3
+#define CCAKE_EOM_MINB 2
 #endif
 template <int D>
 __global__ void __launch_bounds__(128, CCAKE_EOM_MINB)
