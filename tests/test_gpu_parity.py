@@ -184,17 +184,13 @@ def test_runs_are_reproducible():
     assert np.array_equal(res[0][1], res[1][1])
 
 
-def test_full_size_c4_sampled_event_tile():
-    """BASELINE.json configs[3] at full size (1,984,000 particles, the launch configuration bench.py times), checked
-    on a sample the oracle can afford: the event tiles are independent (gaps > 2h + twice the run's reach), so the
-    oracle run on the particles of ONE tile — the very same coordinates and fields, sliced out of the full input —
-    gives the exact expectation for those particles.  Neighbour counts bit-exact, smoothed densities 1e-11 element
-    by element, thermodynamics 1e-11, gradient sums 1e-10, and every evolved field 1e-8 after one RK2 step."""
-    tb = W.make_eos_table(100, 32, with_wq=True)
-    w = W.config_c4(table=tb)
+def _sampled_tile_parity(w, tb, t, nsteps):
+    """GPU on the whole tiled workload, oracle on event tile t alone (the very same coordinates and fields, sliced
+    out of the full input; tiles are independent: gaps > 2h + twice the run's reach).  Neighbour counts bit-exact,
+    smoothed densities 1e-11 element by element, thermodynamics 1e-11, gradient sums 1e-10, and every evolved
+    field 1e-8 after nsteps RK steps (nsteps = 0: one evaluation only)."""
     K = w.meta["tiles"]
     nt = w.n // K
-    t = 7
     sl = slice(t * nt, (t + 1) * nt)
     g = B.from_workload(w)
     o = O.Oracle(**w.params)
@@ -225,9 +221,48 @@ def test_full_size_c4_sampled_event_tile():
     compare(sums, TOL_SUM, "smoothing sums", elementwise=sums)
     compare([B.T, B.P, B.E, B.MU_B, B.MU_S, B.MU_Q], TOL_SUM, "thermodynamics")
     compare(gradient_ids(w.params), TOL_GRAD, "gradient sums")
-    g.step(1)
+    if nsteps:
+        g.step(nsteps)
+        g.synchronize()
+        o.step(nsteps)
+        compare(state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, f"fields after {nsteps} RK2 steps",
+                elementwise=(B.SIGMA_STAR, B.T, B.P))
+    g.close()
+
+
+def test_full_size_c4_sampled_event_tile():
+    """BASELINE.json configs[3] at full size (1,984,000 particles, the launch configuration bench.py times), checked
+    on a sample the oracle can afford: one of its 10 event tiles, one RK2 step."""
+    tb = W.make_eos_table(100, 32, with_wq=True)
+    _sampled_tile_parity(W.config_c4(table=tb), tb, 7, 1)
+
+
+def test_full_size_c3_sampled_event_tile():
+    """BASELINE.json configs[2] at full size (217,156 particles in 4 event tiles): one tile, 3 RK2 steps."""
+    tb = W.make_eos_table(100, 32, with_wq=True)
+    _sampled_tile_parity(W.config_c3(table=tb), tb, 2, 3)
+
+
+def test_full_size_c5_sampled_event_tile():
+    """BASELINE.json configs[4] at full size (19,316,388 particles, 200x48^3 table): one evaluation (all of a1-a7
+    at the loaded state) on one of its 13 event tiles — 1.49 M particles with ~1,700 neighbours each is what the
+    oracle can do in about a minute."""
+    tb = W.make_eos_table(200, 48, with_wq=True)
+    _sampled_tile_parity(W.config_c5(table=tb), tb, 5, 0)
+
+
+def test_full_size_c2():
+    """BASELINE.json configs[1] at full size (40,000 particles, 100x32^3x8 table), whole workload on both sides:
+    one evaluation, then 20 RK2 steps."""
+    w = W.config_c2(nsteps=20)
+    g, o = make_pair(w)
+    assert_cells_equal(g, o)
+    assert_neighbours_equal(g, o)
+    sums = [B.SIGMA_STAR, B.S_STAR, B.RHOSTAR_B, B.RHOSTAR_S, B.RHOSTAR_Q]
+    assert_fields(g, o, sums, TOL_SUM, "smoothing sums", elementwise=sums)
+    g.step(20)
     g.synchronize()
-    o.step(1)
-    compare(state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, "fields after one RK2 step",
-            elementwise=(B.SIGMA_STAR, B.T, B.P))
+    o.step(20)
+    assert_fields(g, o, state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, "fields after 20 steps",
+                  elementwise=(B.SIGMA_STAR, B.T, B.P))
     g.close()
