@@ -52,6 +52,8 @@ struct ccake_ctx {
   double* arena = nullptr;      /* sorted-order doubles */
   ulonglong2* mask_cache = nullptr;   /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
   int mask_tiles = 0;
+  uint32_t *cand_list = nullptr, *cand_cnt = nullptr;   /* per-block candidate lists (optional, as the mask cache) */
+  int cand_cap = 0;
   uint32_t* nnb = nullptr;
   double* theta = nullptr;
   double* scratch = nullptr;    /* N doubles: read_fields staging */
@@ -100,6 +102,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->tot_out); c->tot_out = nullptr;
   cudaFree(c->arena); c->arena = nullptr;
   cudaFree(c->mask_cache); c->mask_cache = nullptr; c->mask_tiles = 0;
+  cudaFree(c->cand_list); c->cand_list = nullptr; cudaFree(c->cand_cnt); c->cand_cnt = nullptr; c->cand_cap = 0;
   cudaFree(c->nnb); c->nnb = nullptr;
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
@@ -153,6 +156,9 @@ void carve(ccake_ctx* c) {
   s.cell_start = c->cell_start;
   s.mask_cache = c->mask_cache;
   s.mask_tiles = c->mask_tiles;
+  s.cand_list = c->cand_list;
+  s.cand_cnt = c->cand_cnt;
+  s.cand_cap = c->cand_cap;
 }
 
 int launch_check(ccake_ctx* c, const char* what) {
@@ -209,6 +215,10 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->grid, c->so);
   if ((rc = mark(c))) return rc;
   /* a4 */
+  if (c->so.cand_cap > 0) {
+    cand_list_kernel<D><<<(int)((N + BH - 1) / BH), BH, 0, st>>>(N, c->grid, c->so);
+    c->launches += 1;
+  }
   launch_smoothing<D>(N, kp, c->grid, c->so, st);
   if ((rc = mark(c))) return rc;
   /* a5 */
@@ -536,6 +546,13 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
       while (tiles > 0 && nblocks * tiles * per_tile > free_b / 8) tiles /= 2;
     if (tiles > 0 && cudaMalloc(&c->mask_cache, nblocks * tiles * per_tile) == cudaSuccess) c->mask_tiles = tiles;
     else { cudaGetLastError(); c->mask_cache = nullptr; c->mask_tiles = 0; }
+    /* candidate lists: CAND_CAP entries per pair block, same policy */
+    int cap = CAND_CAP;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess)
+      while (cap >= 2048 && nblocks * cap * sizeof(uint32_t) > free_b / 8) cap /= 2;
+    if (cap >= 2048 && cudaMalloc(&c->cand_list, nblocks * cap * sizeof(uint32_t)) == cudaSuccess &&
+        cudaMalloc(&c->cand_cnt, nblocks * sizeof(uint32_t)) == cudaSuccess) c->cand_cap = cap;
+    else { cudaGetLastError(); cudaFree(c->cand_list); cudaFree(c->cand_cnt); c->cand_list = c->cand_cnt = nullptr; c->cand_cap = 0; }
   }
   CK(cudaMalloc(&c->nnb, sizeof(uint32_t) * np));
   CK(cudaMalloc(&c->theta, sizeof(double) * np));

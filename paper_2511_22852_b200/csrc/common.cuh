@@ -122,6 +122,11 @@ struct Sorted {
      [pair block][tile number < mask_tiles][stream] x 128 bit; NULL / 0 = no reuse */
   ulonglong2* mask_cache;
   int mask_tiles;
+  /* candidate lists of the pair blocks, written once per substep by cand_list_kernel and read by both passes:
+     block b owns cand_list[b * cand_cap ...], cand_cnt[b] entries (0xffffffff: did not fit, the pass lists its
+     candidates itself); NULL / 0 = not available */
+  uint32_t *cand_list, *cand_cnt;
+  int cand_cap;
 };
 
 /* device-side status counters */
