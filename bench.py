@@ -50,8 +50,8 @@ def flop_grad_per_pair(D, visc, diff):
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# capture of this command (profiles/r1g_README.md); only valid for the workload it was taken on
-NCU_TRAFFIC_BYTES = {("C4", "grad"): 2.077114e9 + 0.471458e9, ("C4", "smooth"): 0.371447e9 + 0.336972e9}
+# capture of this command (profiles/r1j_README.md); only valid for the workload it was taken on
+NCU_TRAFFIC_BYTES = {("C4", "grad"): 2.068537e9 + 0.474270e9, ("C4", "smooth"): 0.538632e9 + 0.310808e9}
 
 
 def make_workload(name, rank=0, tiles=None):
@@ -324,7 +324,7 @@ def run_ours(args):
             "roofline": {"bound": "alu", "kernel": {"grad": "gradient pass a6", "smooth": "smoothing pass a4"}[dom],
                          "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
                          "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)) if args.tiles is None else None,
-                         "traffic_unit": "bytes per launch (ncu --set full, profiles/r1g_README.md)",
+                         "traffic_unit": "bytes per launch (ncu --set full, profiles/r1j_README.md)",
                          "algorithmic_bytes": bytes_pp[dom] * w.n, "peak_source": "fp64 DFMA: 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md)",
                          "flop_per_pair": fg if dom == "grad" else FLOP_SMOOTH_PER_PAIR,
                          "hbm_peak_GBps": hbm, "hbm_peak_source": which},
