@@ -291,6 +291,29 @@ def run_ours(args):
     h2d = 8 * w.n * len(ids)
     d2h = 8 * w.n * len(out_ids)
 
+    # ---- NEXT-1: offline EoS inversion on the device, beside the oracle's on a bounded sample ----
+    eos_inv = None
+    if rank == 0 and w.table is not None and not args.no_cpu:
+        import oracle as O
+        tb = w.table
+        nodes = int(np.prod([len(a) for a in tb["axes"]]))
+        sim.invert_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"])        # warm-up (allocations)
+        t0 = time.perf_counter()
+        sim.invert_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"])        # synchronous: returns with the table installed
+        t_gpu = time.perf_counter() - t0
+        P = O.make_params(**p)
+        rng = np.random.default_rng(7)
+        nsample = 20000
+        ii = [rng.integers(0, len(a), nsample) for a in tb["axes"]]
+        t0 = time.perf_counter()
+        for k in range(nsample):
+            sv = tb["axes"][0][ii[0][k]]
+            O.eos_closed_form(P, sv, [tb["axes"][q + 1][ii[q + 1][k]] * sv for q in range(3)])
+        t_cpu = time.perf_counter() - t0
+        eos_inv = {"nodes": nodes, "columns": len(tb["col_ids"]), "gpu_ms": 1e3 * t_gpu, "gpu_nodes_per_s": nodes / t_gpu,
+                   "cpu_oracle_nodes_per_s": nsample / t_cpu, "cpu_sample": f"{nsample} seeded nodes, 1 thread, through ctypes"}
+        sim.load_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"], torch.as_tensor(tb["data"], device=dev))
+
     if rank == 0:
         hbm, which = peaks()
         nsub = 2 if p["integrator"] == 2 else 4
@@ -334,6 +357,7 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
             "gpu_launches": launches,
+            "eos_inversion": eos_inv,
             "clocks": clocks,
             "status": {"rc": rc, "n_out_of_table": totals[11], "n_bad": totals[13], "x0": totals[0]},
         }

@@ -110,6 +110,18 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
                          const double* const axes[4], int32_t ncols, const int32_t* col_ids,
                          const double* data, int32_t memspace);
 
+/* NEXT-1 of SURVEY.md §8(f): the offline inversion of the equation of state (PAPER.md :576-593, App. A
+ * :2115-2156) done on the device, for the analytic conformal BSQ family of params
+ * (p = c0 T^4 + c2 T^2 sum_q mu_q^2 + c4 sum_q mu_q^4).  For every node of the (s, B, S, Q) grid described by
+ * dims / axis_kind / axes (same meaning as in ccake_load_eos_table; `memspace` says where axes[k] and out live) it
+ * solves (T, mu_q) from (s, n_q) — the cubic of Eq. A.13-A.14 for mu_q(T) inside a bisection in T on the monotone
+ * s(T, mu(T)) — evaluates p, e = 3p, c_s^2 = 1/3, dw/ds and dw/dn_q there, and installs the result as the
+ * context's table exactly as ccake_load_eos_table would.  out may be NULL; otherwise it receives the table,
+ * [d0][d1][d2][d3][ncols] doubles.  Other equations of state are inverted elsewhere and loaded. */
+int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4],
+                           const double* const axes[4], int32_t ncols, const int32_t* col_ids, double* out,
+                           int32_t memspace);
+
 /* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
 int ccake_step(ccake_ctx* c, int32_t nsteps);
 

@@ -28,7 +28,8 @@ RATE = 64
 HOST, DEVICE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_step",
+EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table",
+           "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
            "ccake_last_error"]
@@ -70,6 +71,7 @@ def lib():
         L.ccake_destroy.argtypes = [vp]
         L.ccake_load_particles.argtypes = [vp, i64, i32, C.POINTER(i32), C.POINTER(vp), i32]
         L.ccake_load_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
+        L.ccake_invert_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
         L.ccake_step.argtypes = [vp, i32]
         L.ccake_synchronize.argtypes = [vp]
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
@@ -169,6 +171,19 @@ class Ccake:
             ptrs = (C.c_void_p * 4)(*[a.ctypes.data for a in ax])
         self._chk(lib().ccake_load_eos_table(self._h, dims, kinds, ptrs, len(col_ids), cids, dptr, space),
                   "ccake_load_eos_table")
+
+    def invert_eos_table(self, axes, axis_kind, col_ids, out=False):
+        """ccake_invert_eos_table: build the conformal table on the device and install it; out=True returns it
+        as a numpy array [d0, d1, d2, d3, ncols]."""
+        ax = [np.ascontiguousarray(a, dtype=np.float64) for a in axes]
+        dims = (C.c_int32 * 4)(*[len(a) for a in ax])
+        kinds = (C.c_int32 * 4)(*axis_kind)
+        cids = (C.c_int32 * len(col_ids))(*col_ids)
+        ptrs = (C.c_void_p * 4)(*[a.ctypes.data for a in ax])
+        res = np.empty([len(a) for a in ax] + [len(col_ids)], dtype=np.float64) if out else None
+        self._chk(lib().ccake_invert_eos_table(self._h, dims, kinds, ptrs, len(col_ids), cids,
+                                               res.ctypes.data if out else None, HOST), "ccake_invert_eos_table")
+        return res
 
     def step(self, nsteps=1):
         self._chk(lib().ccake_step(self._h, nsteps), "ccake_step")

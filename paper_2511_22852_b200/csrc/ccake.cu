@@ -660,6 +660,61 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
   return CCAKE_OK;
 }
 
+int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4],
+                           int32_t ncols, const int32_t* col_ids, double* out, int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (!dims || !axis_kind || !axes || !col_ids || ncols <= 0 || ncols > CCAKE_NCOLS_MAX || (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_invert_eos_table";
+    return CCAKE_EINVAL;
+  }
+  int64_t nodes = 1, nax = 0;
+  for (int k = 0; k < 4; ++k) {
+    if (dims[k] < 2 || !axes[k] || (axis_kind[k] != 0 && axis_kind[k] != 1) || (k == 0 && axis_kind[k] != 0)) {
+      c->err = "bad table axis";
+      return CCAKE_EINVAL;
+    }
+    nodes *= dims[k];
+    nax += dims[k];
+  }
+  InvertArgs ia;
+  std::memset(&ia, 0, sizeof(ia));
+  for (int cc = 0; cc < CCAKE_NCOLS_MAX; ++cc) ia.col_of[cc] = -1;
+  for (int k = 0; k < ncols; ++k) {
+    if (col_ids[k] < 0 || col_ids[k] >= CCAKE_NCOLS_MAX) { c->err = "bad column id"; return CCAKE_EINVAL; }
+    ia.col_of[col_ids[k]] = k;
+  }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  double *dax = nullptr, *ddata = nullptr;
+  CK(cudaMalloc(&dax, sizeof(double) * nax));
+  if (cudaMalloc(&ddata, sizeof(double) * nodes * ncols) != cudaSuccess) { cudaFree(dax); c->err = "table allocation"; return CCAKE_ENOMEM; }
+  const double* daxes[4];
+  {
+    int64_t off = 0;
+    for (int k = 0; k < 4; ++k) {
+      cudaMemcpyAsync(dax + off, axes[k], sizeof(double) * dims[k],
+                      memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream);
+      ia.dims[k] = dims[k]; ia.kind[k] = axis_kind[k]; ia.ax[k] = dax + off; daxes[k] = dax + off;
+      off += dims[k];
+    }
+  }
+  ia.ncols = ncols;
+  eos_invert_kernel<<<nblk(nodes, 128), 128, 0, c->stream>>>(c->kp, ia, nodes, ddata);
+  c->launches += 1;
+  int rc = launch_check(c, "eos_invert_kernel");
+  if (rc == CCAKE_OK && cudaStreamSynchronize(c->stream) != cudaSuccess) { c->err = "eos_invert_kernel failed"; rc = CCAKE_ECUDA; }
+  if (rc == CCAKE_OK) rc = ccake_load_eos_table(c, dims, axis_kind, daxes, ncols, col_ids, ddata, CCAKE_DEVICE);
+  if (rc == CCAKE_OK && out)
+    if (cudaMemcpy(out, ddata, sizeof(double) * nodes * ncols,
+                   memspace == CCAKE_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice) != cudaSuccess) {
+      c->err = "copy of the inverted table";
+      rc = CCAKE_ECUDA;
+    }
+  cudaFree(dax);
+  cudaFree(ddata);
+  return rc;
+}
+
 int ccake_step(ccake_ctx* c, int32_t nsteps) {
   if (!c) return CCAKE_EINVAL;
   if (nsteps < 0) { c->err = "nsteps < 0"; return CCAKE_EINVAL; }

@@ -141,6 +141,37 @@ __device__ inline ThermoOut eos_closed_form(const KParams& kp, double s, const d
   return th;
 }
 
+/* NEXT-1: the offline inversion of the EoS table on the device — one thread per node of the
+   (s, B, S, Q) grid; axes 1..3 hold n_q (kind 0) or n_q / s (kind 1).  PAPER.md :576-593, App. A. */
+struct InvertArgs {
+  int dims[4], kind[4], ncols;
+  int col_of[CCAKE_NCOLS_MAX];
+  const double* ax[4];
+};
+__global__ void __launch_bounds__(128)
+eos_invert_kernel(KParams kp, InvertArgs a, int64_t nodes, double* __restrict__ data) {
+  const int64_t node = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (node >= nodes) return;
+  int64_t r = node;
+  const int i3 = (int)(r % a.dims[3]); r /= a.dims[3];
+  const int i2 = (int)(r % a.dims[2]); r /= a.dims[2];
+  const int i1 = (int)(r % a.dims[1]); r /= a.dims[1];
+  const int i0 = (int)r;
+  const double s = a.ax[0][i0];
+  const double y[NQ] = {a.ax[1][i1], a.ax[2][i2], a.ax[3][i3]};
+  double n[NQ];
+  for (int q = 0; q < NQ; ++q) n[q] = (a.kind[q + 1] == 1) ? y[q] * s : y[q];
+  const ThermoOut th = eos_closed_form(kp, s, n);
+  double v[CCAKE_NCOLS_MAX];
+  v[CCAKE_COL_T] = th.T;
+  for (int q = 0; q < NQ; ++q) { v[CCAKE_COL_MUB + q] = th.mu[q]; v[CCAKE_COL_WB + q] = th.wq[q]; }
+  v[CCAKE_COL_P] = th.p; v[CCAKE_COL_CS2] = th.cs2; v[CCAKE_COL_E] = th.e; v[CCAKE_COL_WS] = th.ws;
+  double* __restrict__ o = data + node * a.ncols;
+#pragma unroll
+  for (int c = 0; c < CCAKE_NCOLS_MAX; ++c)
+    if (a.col_of[c] >= 0) o[a.col_of[c]] = v[c];
+}
+
 /* dissipative tensors of one particle: evolved spatial components from the store, time components from
    u_mu pi^{mu nu} = 0 and u_mu J^mu = 0 (never evolved; DESIGN reading 13) */
 struct Dissip { double pit[4][4], Jt[NQ][4], bulkt; };
