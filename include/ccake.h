@@ -48,6 +48,10 @@ enum {
   CCAKE_MASS = 26,                            /* SPH weight m_b (default 1, Eq. 75 :898)                       */
   CCAKE_WORK = 27,                            /* accumulated longitudinal work (2+1D hyperbolic), starts at 0  */
   CCAKE_NSTATE = 28,
+  /* applicability diagnostics of PAPER.md Eq. 58-61 (:797-805), read only, evaluated at the current state:
+     Kn_pi = tau_pi sqrt(sigma^{mn} sigma_{mn}), Re_pi^-1 = sqrt(pi^{mn} pi_{mn}) / p, Kn_Pi = tau_Pi theta,
+     Re_Pi^-1 = |Pi| / p */
+  CCAKE_KN_PI = 28, CCAKE_RE_PI, CCAKE_KN_BULK, CCAKE_RE_BULK,
   CCAKE_SIGMA_STAR = 32, CCAKE_S_DENS, CCAKE_RHO_B, CCAKE_RHO_S, CCAKE_RHO_Q,  /* sigma*, rest-frame s, n_q   */
   CCAKE_T, CCAKE_MU_B, CCAKE_MU_S, CCAKE_MU_Q,
   CCAKE_P = 41, CCAKE_E, CCAKE_CS2, CCAKE_GAMMA, CCAKE_NNB, CCAKE_CELL, CCAKE_THETA, CCAKE_SIGMA, CCAKE_S_STAR,

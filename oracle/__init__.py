@@ -17,6 +17,7 @@ JB1, JB2, JB3, JS1, JS2, JS3, JQ1, JQ2, JQ3 = range(17, 26)
 MASS, WORK, NSTATE = 26, 27, 28
 SIGMA_STAR, S_DENS, RHO_B, RHO_S, RHO_Q, T, MU_B, MU_S, MU_Q = range(32, 41)
 P, E, CS2, GAMMA, NNB, CELL, THETA, SIGMA, S_STAR = range(41, 50)
+KN_PI, RE_PI, KN_BULK, RE_BULK = range(28, 32)      # applicability diagnostics, Eq. 58-61
 RHOSTAR_B, RHOSTAR_S, RHOSTAR_Q, WS, DIVV = range(50, 55)
 FM1, FM2, FM3, FK_B, FK_S, FK_Q = range(55, 61)
 RATE = 64

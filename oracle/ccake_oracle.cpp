@@ -13,6 +13,7 @@
  *                                         Eq. 87-104 :964-1041
  *   Step 6  integrator                    not in the paper (DESIGN reading 7): RK2 midpoint / classical RK4
  *   Step 7  conserved totals              §5.6.5 :1049-1063
+ *   extra   applicability diagnostics     Eq. 58-61 :797-805 (Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1; pinned on Bjorken)
  *
  * There is no blocking, fusion or reordering: loops are gather form (for a { for b }), the per-particle linear
  * system in the unknown time derivatives is written LITERALLY in covariant form with generic 4x4 metric and
@@ -77,6 +78,7 @@ struct Derived {
   std::vector<double> sigma_star, s_star, rho_star[NQ], gamma, sigma, s, n[NQ];
   std::vector<Thermo> th;
   std::vector<double> theta, divv, fm[3], fk[NQ];
+  std::vector<double> diag[4];       /* Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1 (Eq. 58-61) */
   std::vector<double> cell, nnb;
   /* per-particle pair inputs (Step 5): P/sigma*^2, B^j_i/sigma*^2, K^j_q/sigma*^2, alpha_q, v^i */
   std::vector<double> Ppair, Bpair[3][3], Kpair[NQ][3], alpha[NQ], v[3];
@@ -661,7 +663,7 @@ static int state_id_of_pi(int i, int j) {
 /* Assemble and solve the linear system of one particle; write the time derivatives into k.
    Returns false on a singular system. */
 static bool eom_particle(const oracle_params& P, const Geometry& g, const State& y, const Derived& d, int64_t a,
-                         double x0, State& k, double& theta_out) {
+                         double x0, State& k, double& theta_out, double diag_out[4]) {
   const int D = P.dim;
   const Unknowns U = unknown_layout(D);
   const int NU = U.nu;
@@ -764,7 +766,7 @@ static bool eom_particle(const oracle_params& P, const Geometry& g, const State&
      sigma^{mn} = 1/2 (nabla^m u^n + nabla^n u^m) - 1/2 (u^m Du^n + u^n Du^m) - 1/3 Delta^{mn} theta
      omega^{mn} = 1/2 (nabla^m u^n - nabla^n u^m) - 1/2 (u^m Du^n - u^n Du^m)                          */
   Aff sg[4][4], om[4][4];
-  if (shear || bulk) {
+  {   /* always: the diagnostics of Eq. 58 need sigma^{mn} also for an ideal fluid */
     for (int m = 0; m < 4; ++m)
       for (int n = 0; n < 4; ++n) {
         const Aff up_mn = g.gup[m] * CD[m][n], up_nm = g.gup[n] * CD[n][m];
@@ -933,6 +935,21 @@ static bool eom_particle(const oracle_params& P, const Geometry& g, const State&
   if (P.coords == 1 && D == 2)
     k.f[OF_WORK][a] = (y.f[OF_MASS][a] / d.sigma_star[a]) * (th.p + Pi + x0 * x0 * sig * ds.pit[3][3]);
   theta_out = eval(theta, X, NU);
+  /* applicability diagnostics at the solution, Eq. 58-61 (:797-805); the metric is diagonal, so
+     A^{mn} A_{mn} = sum_mn g_mm g_nn (A^{mn})^2 */
+  {
+    double ss = 0.0, pp = 0.0;
+    for (int m = 0; m < 4; ++m)
+      for (int n = 0; n < 4; ++n) {
+        const double sv = eval(sg[m][n], X, NU), pv = sig * ds.pit[m][n];
+        ss += g.glo[m] * g.glo[n] * sv * sv;
+        pp += g.glo[m] * g.glo[n] * pv * pv;
+      }
+    diag_out[0] = tr.tau_pi * std::sqrt(std::max(ss, 0.0));
+    diag_out[1] = std::sqrt(std::max(pp, 0.0)) / th.p;
+    diag_out[2] = tr.tau_Pi * theta_out;
+    diag_out[3] = std::fabs(Pi) / th.p;
+  }
   return true;
 }
 
@@ -958,14 +975,16 @@ static int evaluate(oracle_ctx* c, const State& y, double x0, Derived& d, State&
   const Geometry g = geometry(P, x0);
   for (int f = 0; f < OF_NSTATE; ++f) k.f[f].assign(N, 0.0);
   d.theta.assign(N, 0.0);
+  for (int i = 0; i < 4; ++i) d.diag[i].assign(N, 0.0);
   for (int i = 0; i < 3; ++i) d.fm[i].assign(N, 0.0);
   for (int q = 0; q < NQ; ++q) d.fk[q].assign(N, 0.0);
   int bad = 0;
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : bad)
   for (int64_t a = 0; a < N; ++a) {
-    double th = 0.0;
-    if (!eom_particle(P, g, y, d, a, x0, k, th)) bad++;
+    double th = 0.0, dg[4] = {0.0, 0.0, 0.0, 0.0};
+    if (!eom_particle(P, g, y, d, a, x0, k, th, dg)) bad++;
     d.theta[a] = th;
+    for (int i = 0; i < 4; ++i) d.diag[i][a] = dg[i];
     for (int i = 0; i < P.dim; ++i) d.fm[i][a] = g.sqrtg * (d.FP[i][a] - d.FB[i][a]);
     for (int q = 0; q < NQ; ++q) d.fk[q][a] = -g.sqrtg * d.FK[q][a];
   }
@@ -1145,6 +1164,10 @@ int oracle_read_fields(oracle_ctx* c, int32_t nfields, const int32_t* ids, doubl
       case OF_NNB: src = &d.nnb; break;
       case OF_CELL: src = &d.cell; break;
       case OF_THETA: src = &d.theta; break;
+      case OF_KN_PI: src = &d.diag[0]; break;
+      case OF_RE_PI: src = &d.diag[1]; break;
+      case OF_KN_BULK: src = &d.diag[2]; break;
+      case OF_RE_BULK: src = &d.diag[3]; break;
       case OF_SIGMA: src = &d.sigma; break;
       case OF_S_STAR: src = &d.s_star; break;
       case OF_RHOSTAR_B: src = &d.rho_star[0]; break;

@@ -28,6 +28,9 @@ enum {
   OF_PI11, OF_PI12, OF_PI13, OF_PI22, OF_PI23, OF_PI33,
   OF_JB1, OF_JB2, OF_JB3, OF_JS1, OF_JS2, OF_JS3, OF_JQ1, OF_JQ2, OF_JQ3,
   OF_MASS = 26, OF_WORK = 27, OF_NSTATE = 28,
+  /* applicability diagnostics, Eq. 58-61 (:797-805): Kn_pi = tau_pi sqrt(sigma^{mn} sigma_{mn}),
+     Re_pi^-1 = sqrt(pi^{mn} pi_{mn}) / p, Kn_Pi = tau_Pi theta, Re_Pi^-1 = |Pi| / p; read only */
+  OF_KN_PI = 28, OF_RE_PI, OF_KN_BULK, OF_RE_BULK,
   /* derived, read only; evaluated at the current state */
   OF_SIGMA_STAR = 32, OF_S_DENS, OF_RHO_B, OF_RHO_S, OF_RHO_Q, OF_T, OF_MU_B, OF_MU_S, OF_MU_Q,
   OF_P = 41, OF_E, OF_CS2, OF_GAMMA, OF_NNB, OF_CELL, OF_THETA, OF_SIGMA, OF_S_STAR,

@@ -50,6 +50,7 @@ struct ccake_ctx {
   double *tot_partial = nullptr, *tot_out = nullptr;
   int tot_blocks = 0;
   double* arena = nullptr;      /* sorted-order doubles */
+  double* diag = nullptr;       /* 4 x npad: applicability diagnostics of the latest refresh (sorted order) */
   ulonglong2* mask_cache = nullptr;   /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
   int mask_tiles = 0;
   uint32_t *cand_list = nullptr, *cand_cnt = nullptr;   /* per-block candidate lists (optional, as the mask cache) */
@@ -101,6 +102,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->tot_partial); c->tot_partial = nullptr;
   cudaFree(c->tot_out); c->tot_out = nullptr;
   cudaFree(c->arena); c->arena = nullptr;
+  cudaFree(c->diag); c->diag = nullptr;
   cudaFree(c->mask_cache); c->mask_cache = nullptr; c->mask_tiles = 0;
   cudaFree(c->cand_list); c->cand_list = nullptr; cudaFree(c->cand_cnt); c->cand_cnt = nullptr; c->cand_cap = 0;
   cudaFree(c->nnb); c->nnb = nullptr;
@@ -232,7 +234,8 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   RkArgs rk = rk_in;
   rk.Ycur = Ycur;
   rk.theta_out = c->theta;
-  eom_kernel<D><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
+  if (rk.diag) eom_kernel<D, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
+  else eom_kernel<D, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
   if ((rc = mark(c))) return rc;
   c->launches += 5;
   return launch_check(c, "substep");
@@ -311,6 +314,8 @@ int refresh(ccake_ctx* c) {
   std::memset(&rk, 0, sizeof(rk));
   rk.update = 0;
   rk.Krate = c->Krate;
+  if (!c->diag) CK(cudaMalloc(&c->diag, sizeof(double) * c->npad * 4));
+  rk.diag = c->diag;
   double* Ycur = c->Y[0];
   int rc = build_cells(c, Ycur, true);
   if (!rc) {
@@ -782,6 +787,9 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
       case CCAKE_CS2: src_sorted = so.cs2; break;
       case CCAKE_GAMMA: src_sorted = so.gamma; break;
       case CCAKE_THETA: src_sorted = c->theta; break;
+      case CCAKE_KN_PI: case CCAKE_RE_PI: case CCAKE_KN_BULK: case CCAKE_RE_BULK:
+        src_sorted = c->diag + (int64_t)(id - CCAKE_KN_PI) * np;
+        break;
       case CCAKE_SIGMA: src_sorted = so.sigma; break;
       case CCAKE_S_STAR: src_sorted = so.s_star; break;
       case CCAKE_RHOSTAR_B: src_sorted = so.rho_star[0]; break;

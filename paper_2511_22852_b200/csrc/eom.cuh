@@ -48,7 +48,7 @@ struct EomOut {
 
 template <int D>
 __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
-                                       EomOut& o) {
+                                          EomOut& o, double* sgsq_out = nullptr) {
   const double gam = in.gam, sig = in.sig;
   const double igam = in.igam, itau = in.itau;
   double du[4], dulo[4];
@@ -72,7 +72,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
   for (int n = 0; n < 4; ++n) { CD[0][n] += du[n]; Du[n] = in.Duc[n] + gam * du[n]; Dulo[n] = in.glo[n] * Du[n]; }
 
   const double Pi = in.ds.bulkt * sig;
-  const bool need_sg = kp.shear || (kp.bulk && in.lambda_Pipi != 0.0);
+  const bool need_sg = kp.shear || (kp.bulk && in.lambda_Pipi != 0.0) || sgsq_out != nullptr;
   double sg[4][4];
   if (need_sg) {
 #pragma unroll
@@ -84,6 +84,14 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
                          (Delta * (1.0 / 3.0)) * theta;
         sg[m][n] = v; sg[n][m] = v;
       }
+  }
+  if (sgsq_out) {                                  /* sigma^{mn} sigma_{mn} for Eq. 58 (diagonal metric) */
+    double ss = 0.0;
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = 0; n < 4; ++n) ss += in.glo[m] * in.glo[n] * sg[m][n] * sg[m][n];
+    *sgsq_out = ss;
   }
   /* bulk */
   o.dBulk = 0.0;
@@ -243,6 +251,7 @@ struct RkArgs {
   double* Yacc;         /* RK4 accumulator or NULL                 */
   double* Krate;        /* rates in store order, or NULL           */
   double* theta_out;    /* sorted order                            */
+  double* diag;         /* 4 x npad, sorted order: Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1 (DIAG kernels only) */
   double c_out, w_acc;
   int acc_mode;         /* 0 none | 1 set | 2 add | 3 final        */
   int update;           /* 0: rates only (refresh)                 */
@@ -251,7 +260,7 @@ struct RkArgs {
 #ifndef CCAKE_EOM_MINB
 #define CCAKE_EOM_MINB 2
 #endif
-template <int D>
+template <int D, bool DIAG>
 __global__ void __launch_bounds__(128, CCAKE_EOM_MINB)
 eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, uint32_t field_mask,
            Status* __restrict__ status) {
@@ -422,7 +431,19 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       for (int k = r + 1; k < D; ++k) s0 -= M[r][k] * du[k];
       du[r] = s0 / M[r][r];
     }
-  eom_rates<D>(kp, gm, in, du, o);
+  double sgsq = 0.0;
+  eom_rates<D>(kp, gm, in, du, o, DIAG ? &sgsq : nullptr);
+  if (DIAG) {                                      /* applicability diagnostics, Eq. 58-61 (:797-805) */
+    double pp = 0.0;
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = 0; n < 4; ++n) { const double pv = in.sig * in.ds.pit[m][n]; pp += in.glo[m] * in.glo[n] * pv * pv; }
+    rk.diag[0 * npad + i] = in.tau_pi * sqrt(fmax(sgsq, 0.0));
+    rk.diag[1 * npad + i] = sqrt(fmax(pp, 0.0)) / in.p;
+    rk.diag[2 * npad + i] = in.tau_Pi * o.theta;
+    rk.diag[3 * npad + i] = fabs(in.ds.bulkt * in.sig) / in.p;
+  }
   if (!ok || !(o.dS == o.dS) || !(du[0] == du[0])) atomicAdd(&status->n_bad, 1ULL);
 
   /* rates of the evolved set */

@@ -266,3 +266,20 @@ def test_full_size_c2():
     assert_fields(g, o, state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, "fields after 20 steps",
                   elementwise=(B.SIGMA_STAR, B.T, B.P))
     g.close()
+
+
+@pytest.mark.parametrize("name", ["C3_small", "C4_small", "cloud2_hyp_dnmr", "cloud3_hyp_is", "cloud3_cart_closed"])
+def test_applicability_diagnostics(name):
+    """NEXT-4 of SURVEY.md §8(f), Eq. 58-61 (:797-805): Knudsen and inverse Reynolds numbers of shear and
+    bulk per particle, at the loaded state and after 3 RK steps — 1e-9 of the field's infinity norm (they are built
+    from the velocity-gradient sums, tolerance class of gradient_ids)."""
+    w = WORKLOADS[name]()
+    g, o = make_pair(w)
+    ids = [B.KN_PI, B.RE_PI, B.KN_BULK, B.RE_BULK]
+    assert (B.KN_PI, B.RE_PI, B.KN_BULK, B.RE_BULK) == (O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK)
+    assert_fields(g, o, ids, 1e-9, "diagnostics at the loaded state")
+    g.step(3)
+    g.synchronize()
+    o.step(3)
+    assert_fields(g, o, ids, 1e-8, "diagnostics after 3 steps")
+    g.close()

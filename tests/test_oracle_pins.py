@@ -673,3 +673,53 @@ def test_kappa_matrix_golden(golden_dir):
     rows = read_golden_table(os.path.join(golden_dir, "kappa_over_T2.txt"))
     flat = [float(v) for r in rows[:3] for v in r]
     assert flat == W.KAPPA_OVER_T2 and [float(v) for v in rows[3]] == W.TAU_Q_TIMES_T
+
+
+def test_applicability_diagnostics_on_bjorken():
+    """PAPER.md Eq. 58-61 (:797-805) on the boost-invariant slab at rest in hyperbolic coordinates, where
+    everything is closed form: theta = 1/tau and sigma^{mu nu} sigma_{mu nu} = 2/(3 tau^2)
+    (sigma^{xx} = sigma^{yy} = 1/(3 tau), sigma^{eta eta} = -2/(3 tau^3)), so Kn_pi = tau_pi sqrt(2/3) / tau and
+    Kn_Pi = tau_Pi / tau; with u = (1,0,0,0), pi^{0 mu} = 0 and pi^{mu nu} pi_{mu nu} =
+    sigma^2 (PI11^2 + PI22^2 + 2 PI12^2 + tau^4 PI33^2), Re_Pi^-1 = |BULK sigma| / p.  A dropped metric factor, a
+    missing 1/3 Delta theta or a wrong relaxation time fails one of these."""
+    n, dx, h, tau0 = 36, 0.1, 0.3, 0.7
+    x1 = (np.arange(n) - 0.5 * (n - 1)) * dx
+    X, Y = np.meshgrid(x1, x1)
+    x, y = X.ravel(), Y.ravel()
+    T0 = 0.30 / W.HBARC
+    p = W.base_params(dim=2, coords=1, eom=1, flags=3, eos_kind=0, h=h, x0_start=tau0, dx0=0.01, eta_over_s=0.2,
+                      zeta_max=0.1, tau_Pi_coeff=1.5)
+    N = x.size
+    pi11, pi22, pi12, pi33, bulk = 0.013, -0.004, 0.002, -0.009 / tau0 ** 2, -0.006
+    o = O.Oracle(**p)
+    o.load_particles({O.R1: x, O.R2: y, O.S: np.full(N, 4 * C0 * T0 ** 3 * tau0 * dx * dx),
+                      O.PI11: np.full(N, pi11), O.PI22: np.full(N, pi22), O.PI12: np.full(N, pi12),
+                      O.PI33: np.full(N, pi33), O.BULK: np.full(N, bulk)})
+    ic = int(np.argmin(x * x + y * y))
+    f = o.read_fields([O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK, O.THETA, O.SIGMA, O.P, O.T, O.S_DENS, O.E])
+    T, s, e, pr, sig = (f[k][ic] for k in (O.T, O.S_DENS, O.E, O.P, O.SIGMA))
+    eta = p["eta_over_s"] * s
+    tau_pi = max(p["tau_pi_coeff"] * eta / (e + pr), p["tau_floor"])
+    tau_Pi = p["tau_Pi_coeff"] * tau_pi
+    assert abs(f[O.THETA][ic] * tau0 - 1) < 1e-6
+    assert abs(f[O.KN_PI][ic] / (tau_pi * np.sqrt(2.0 / 3.0) / tau0) - 1) < 1e-6
+    assert abs(f[O.KN_BULK][ic] / (tau_Pi / tau0) - 1) < 1e-6
+    pipi = sig ** 2 * (pi11 ** 2 + pi22 ** 2 + 2 * pi12 ** 2 + tau0 ** 4 * pi33 ** 2)
+    assert abs(f[O.RE_PI][ic] / (np.sqrt(pipi) / pr) - 1) < 1e-12
+    assert abs(f[O.RE_BULK][ic] / (abs(bulk * sig) / pr) - 1) < 1e-12
+
+
+def test_applicability_diagnostics_vanish_for_uniform_fluid_at_rest():
+    """Cartesian, uniform, at rest, no dissipative fields: sigma^{mu nu} = 0, theta = 0, pi = Pi = 0 in the interior,
+    so all four numbers vanish (to the SPH noise of the velocity gradient, which is exactly 0 for u = 0)."""
+    n, dx = 30, 0.1
+    x1 = (np.arange(n) - 0.5 * (n - 1)) * dx
+    X, Y = np.meshgrid(x1, x1)
+    x, y = X.ravel(), Y.ravel()
+    p = W.base_params(dim=2, coords=0, eom=1, flags=3, eos_kind=0, h=0.3, x0_start=1.0, dx0=0.01, eta_over_s=0.2)
+    o = O.Oracle(**p)
+    o.load_particles({O.R1: x, O.R2: y, O.S: np.full(x.size, 4 * C0 * (0.3 / W.HBARC) ** 3 * dx * dx)})
+    ic = int(np.argmin(x * x + y * y))
+    f = o.read_fields([O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK])
+    for k in (O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK):
+        assert abs(f[k][ic]) < 1e-12
