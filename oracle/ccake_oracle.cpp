@@ -79,6 +79,7 @@ struct Derived {
   std::vector<Thermo> th;
   std::vector<double> theta, divv, fm[3], fk[NQ];
   std::vector<double> diag[4];       /* Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1 (Eq. 58-61) */
+  std::vector<double> fo[9];         /* d_mu eps (4), n_mu (4), |d sigma| (Eq. 145-148) */
   std::vector<double> cell, nnb;
   /* per-particle pair inputs (Step 5): P/sigma*^2, B^j_i/sigma*^2, K^j_q/sigma*^2, alpha_q, v^i */
   std::vector<double> Ppair, Bpair[3][3], Kpair[NQ][3], alpha[NQ], v[3];
@@ -953,6 +954,47 @@ static bool eom_particle(const oracle_params& P, const Geometry& g, const State&
   return true;
 }
 
+/* ------------------------------------------------------------------------ freeze-out element (§5.10) ---- */
+/* PAPER.md Eq. 145-148 (:1466-1482), per particle at the current state, given the rates k = dy/dx0 of Step 5:
+     d_i eps   = (1/sigma*_a) sum_b m_b (eps_b - eps_a) d_i W_ab        ("derivatives ... using the SPH method", n = +1 form)
+     d eps/dx0 = T ds/dx0 + mu_q dn_q/dx0 along the particle (first law), with s = S sigma, n_q = N_q sigma and
+                 d sigma/dx0 = -sigma theta / gamma (D sigma = -sigma theta)
+     d_0 eps   = d eps/dx0 - v^i d_i eps                                 (Eulerian time derivative)
+     n_mu      = -d_mu eps / sqrt|d_mu eps d^mu eps|,   |d sigma| = m / (sigma |u^mu n_mu|)                       */
+static void freezeout_element(const oracle_params& P, const Geometry& g, const State& y, const State& k, int64_t N,
+                              Derived& d) {
+  const int D = P.dim;
+  for (int i = 0; i < 9; ++i) d.fo[i].assign(N, 0.0);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t a = 0; a < N; ++a) {
+    double de[4] = {0, 0, 0, 0};
+    for (int64_t kk = d.nb_off[a]; kk < d.nb_off[a + 1]; ++kk) {
+      const int64_t b = d.nb_idx[kk];
+      double dr[3] = {0, 0, 0}, gW[3];
+      for (int i = 0; i < D; ++i) dr[i] = y.f[OF_R1 + i][a] - y.f[OF_R1 + i][b];
+      kernel_gradW(D, P.h, dr, gW);
+      for (int i = 0; i < D; ++i) de[1 + i] += y.f[OF_MASS][b] * (d.th[b].e - d.th[a].e) * gW[i];
+    }
+    for (int i = 0; i < D; ++i) de[1 + i] /= d.sigma_star[a];
+    double u[4];
+    four_velocity(P, g, y, a, u);
+    const double gam = u[0], sig = d.sigma[a], th_ = d.theta[a];
+    const Thermo& th = d.th[a];
+    const double dsig = -sig * th_ / gam;
+    double deps = th.T * (sig * k.f[OF_S][a] + y.f[OF_S][a] * dsig);
+    for (int q = 0; q < NQ; ++q) deps += th.mu[q] * (sig * k.f[OF_NB + q][a] + y.f[OF_NB + q][a] * dsig);
+    de[0] = deps;
+    for (int i = 1; i <= D; ++i) de[0] -= (u[i] / gam) * de[i];
+    double nn = 0.0;
+    for (int m = 0; m < 4; ++m) nn += g.gup[m] * de[m] * de[m];
+    const double norm = std::sqrt(std::fabs(nn));
+    double un = 0.0, nmu[4];
+    for (int m = 0; m < 4; ++m) { nmu[m] = (norm > 0.0) ? -de[m] / norm : 0.0; un += u[m] * nmu[m]; }
+    for (int m = 0; m < 4; ++m) { d.fo[m][a] = de[m]; d.fo[4 + m][a] = nmu[m]; }
+    d.fo[8][a] = (un != 0.0) ? y.f[OF_MASS][a] / (sig * std::fabs(un)) : 0.0;
+  }
+}
+
 /* f(y, x0): all of Steps 1-5 */
 static double now_s() {
   return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
@@ -1046,6 +1088,7 @@ static int refresh(oracle_ctx* c) {
   if (c->derived_valid) return ORACLE_OK;
   int rc = evaluate(c, c->y, c->x0, c->d, c->rate);
   if (rc) return rc;
+  freezeout_element(c->P, geometry(c->P, c->x0), c->y, c->rate, c->N, c->d);
   c->derived_valid = true;
   return ORACLE_OK;
 }
@@ -1164,6 +1207,8 @@ int oracle_read_fields(oracle_ctx* c, int32_t nfields, const int32_t* ids, doubl
       case OF_NNB: src = &d.nnb; break;
       case OF_CELL: src = &d.cell; break;
       case OF_THETA: src = &d.theta; break;
+      case OF_FO_DE0: case OF_FO_DE1: case OF_FO_DE2: case OF_FO_DE3: case OF_FO_N0: case OF_FO_N1: case OF_FO_N2:
+      case OF_FO_N3: case OF_FO_DSIGMA: src = &d.fo[id - OF_FO_DE0]; break;
       case OF_KN_PI: src = &d.diag[0]; break;
       case OF_RE_PI: src = &d.diag[1]; break;
       case OF_KN_BULK: src = &d.diag[2]; break;

@@ -38,7 +38,11 @@ enum {
   OF_FM1 = 55, OF_FM2, OF_FM3,   /* sqrt(-g) (FP_i - FB_i): right-hand side of the momentum equation */
   OF_FK_B = 58, OF_FK_S, OF_FK_Q, /* -sqrt(-g) FK_q: right-hand side of the charge equation           */
   /* OF_RATE + state id: d(state field)/dx0 at the current state */
-  OF_RATE = 64
+  OF_RATE = 64,
+  /* freeze-out surface element of PAPER.md §5.10, Eq. 145-148 (:1466-1482), per particle at the current state:
+     d_mu eps (mu = 0..3), the outward unit normal n_mu = -d_mu eps / sqrt|d eps . d eps| and
+     |d sigma| = m / (sigma |u^mu n_mu|); read only */
+  OF_FO_DE0 = 96, OF_FO_DE1, OF_FO_DE2, OF_FO_DE3, OF_FO_N0, OF_FO_N1, OF_FO_N2, OF_FO_N3, OF_FO_DSIGMA
 };
 
 typedef struct oracle_params {

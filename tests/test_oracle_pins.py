@@ -723,3 +723,59 @@ def test_applicability_diagnostics_vanish_for_uniform_fluid_at_rest():
     f = o.read_fields([O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK])
     for k in (O.KN_PI, O.RE_PI, O.KN_BULK, O.RE_BULK):
         assert abs(f[k][ic]) < 1e-12
+
+
+def test_freezeout_element_on_bjorken():
+    """PAPER.md Eq. 145-148 (:1466-1482) where everything is closed form — the boost-invariant ideal slab at rest in
+    hyperbolic coordinates: d_i eps = 0, d_tau eps = -(eps + p)/tau (so the surface is space-like, n_mu =
+    (+1, 0, 0, 0): the outward normal of a cooling fluid points to later times), u.n = 1 and
+    |d sigma| = m / sigma.  A wrong sign in Eq. 147, a missing D sigma = -sigma theta or a rate taken per unit of
+    proper time fails this."""
+    p, ic, Tini, tau0, tau1, _ = _bjorken_run(0, 0.01, 0, eom=0)
+    n, dx = 36, 0.1
+    x1 = (np.arange(n) - 0.5 * (n - 1)) * dx
+    X, Y = np.meshgrid(x1, x1)
+    o = O.Oracle(**p)
+    T0 = 0.30 / W.HBARC
+    o.load_particles({O.R1: X.ravel(), O.R2: Y.ravel(), O.S: np.full(X.size, 4 * C0 * T0 ** 3 * tau0 * dx * dx)})
+    ids = [O.FO_DE0, O.FO_DE1, O.FO_DE2, O.FO_DE3, O.FO_N0, O.FO_N1, O.FO_N2, O.FO_N3, O.FO_DSIGMA, O.E, O.P, O.SIGMA]
+    f = {k: v[ic] for k, v in o.read_fields(ids).items()}
+    assert abs(f[O.FO_DE0] / (-(f[O.E] + f[O.P]) / tau0) - 1) < 1e-6
+    assert abs(f[O.FO_DE1]) < 1e-9 * abs(f[O.FO_DE0]) and abs(f[O.FO_DE2]) < 1e-9 * abs(f[O.FO_DE0]) and f[O.FO_DE3] == 0.0
+    assert abs(f[O.FO_N0] - 1.0) < 1e-12 and abs(f[O.FO_N1]) < 1e-9 and abs(f[O.FO_N2]) < 1e-9
+    assert abs(f[O.FO_DSIGMA] * f[O.SIGMA] - 1.0) < 1e-12          # m = 1
+
+
+def test_freezeout_normal_on_gubser():
+    """Ideal Gubser flow (Eq. 116-120): eps = 3 c0 T(tau, r)^4 is analytic, so d_mu eps is too.  At r = 1.55 fm the
+    SPH values converge to the analytic ones at second order in h (h = 0.3 -> 0.15 with dx = h/3: errors of ~9 % and
+    ~2.5 % of d_tau eps and d_r eps, ratio > 3), the gradient is radial, the normal is unit (n.n = +-1), and
+    |d sigma| = m / (sigma |u.n|) agrees with the analytic normal to the same accuracy."""
+    errs = []
+    for n, dx, h in ((80, 0.1, 0.3), (160, 0.05, 0.15)):
+        w = W.config_c1(hyperbolic=True, n=n, dx=dx)
+        p = dict(w.params)
+        p["h"] = h
+        o = O.Oracle(**p)
+        o.load_particles(w.fields)
+        x, y = w.fields[O.R1], w.fields[O.R2]
+        r = np.hypot(x, y)
+        ia = int(np.argmin(np.abs(x - 1.55) + np.abs(y - 0.05)))
+        ids = [O.FO_DE0, O.FO_DE1, O.FO_DE2, O.FO_N0, O.FO_N1, O.FO_N2, O.FO_DSIGMA, O.SIGMA]
+        f = {k: v[ia] for k, v in o.read_fields(ids).items()}
+        tau, ra, eps_ = 1.0, r[ia], 1e-5
+        e = lambda t, rr: 3 * C0 * W.gubser_T(t, rr) ** 4
+        de_t = (e(tau + eps_, ra) - e(tau - eps_, ra)) / (2 * eps_)
+        de_r = (e(tau, ra + eps_) - e(tau, ra - eps_)) / (2 * eps_)
+        der = (f[O.FO_DE1] * x[ia] + f[O.FO_DE2] * y[ia]) / ra
+        errs.append((abs(f[O.FO_DE0] / de_t - 1), abs(der / de_r - 1)))
+        assert abs(f[O.FO_DE1] * y[ia] - f[O.FO_DE2] * x[ia]) < 1e-3 * abs(de_r) * ra          # radial
+        nn = f[O.FO_N0] ** 2 - f[O.FO_N1] ** 2 - f[O.FO_N2] ** 2
+        assert abs(abs(nn) - 1) < 1e-12
+        norm = np.sqrt(abs(de_t ** 2 - de_r ** 2))
+        n0, nr = -de_t / norm, -de_r / norm
+        ur = W.gubser_ur(tau, ra)
+        un = np.sqrt(1 + ur ** 2) * n0 + ur * nr
+        assert abs(f[O.FO_DSIGMA] * f[O.SIGMA] * abs(un) - 1) < (0.25 if h > 0.2 else 0.07)
+    assert errs[0][0] < 0.12 and errs[0][1] < 0.12 and errs[1][0] < 0.03 and errs[1][1] < 0.03
+    assert errs[0][0] / errs[1][0] > 3.0 and errs[0][1] / errs[1][1] > 3.0
