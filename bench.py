@@ -314,6 +314,19 @@ def run_ours(args):
                    "cpu_oracle_nodes_per_s": nsample / t_cpu, "cpu_sample": f"{nsample} seeded nodes, 1 thread, through ctypes"}
         sim.load_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"], torch.as_tensor(tb["data"], device=dev))
 
+    # ---- NEXT-2: freeze-out element pass (one more pair pass over the cached lists and masks), device buffers ----
+    fo_ms = None
+    if rank == 0:
+        buf = torch.empty(w.n, dtype=torch.float64, device=dev)
+        sim.read_fields([B.T], out=[buf])                                 # refresh of the derived fields
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            f0.record()
+            sim.read_fields([B.FO_DSIGMA], out=[buf])
+            f1.record()
+        torch.cuda.synchronize()
+        fo_ms = f0.elapsed_time(f1)
+
     if rank == 0:
         hbm, which = peaks()
         nsub = 2 if p["integrator"] == 2 else 4
@@ -358,6 +371,7 @@ def run_ours(args):
                     "steps": e2e_steps},
             "gpu_launches": launches,
             "eos_inversion": eos_inv,
+            "freezeout_element_ms": fo_ms,
             "clocks": clocks,
             "status": {"rc": rc, "n_out_of_table": totals[11], "n_bad": totals[13], "x0": totals[0]},
         }

@@ -58,7 +58,12 @@ enum {
   CCAKE_RHOSTAR_B = 50, CCAKE_RHOSTAR_S, CCAKE_RHOSTAR_Q, CCAKE_WS, CCAKE_DIVV,
   CCAKE_FM1 = 55, CCAKE_FM2, CCAKE_FM3,       /* right-hand side of the momentum equation, sqrt(-g)(FP_i - FB_i) */
   CCAKE_FK_B = 58, CCAKE_FK_S, CCAKE_FK_Q,    /* right-hand side of the charge equation, -sqrt(-g) FK_q         */
-  CCAKE_RATE = 64                             /* CCAKE_RATE + state id: d(state field)/dx0 at the current state */
+  CCAKE_RATE = 64,                            /* CCAKE_RATE + state id: d(state field)/dx0 at the current state */
+  /* NEXT-2 of SURVEY.md §8(f): freeze-out surface element of PAPER.md §5.10, Eq. 145-148 (:1466-1482), per particle
+     at the current state: d_mu eps (mu = 0..3; SPH n = +1 derivative in space, first law + rates in time), the
+     outward unit normal n_mu = -d_mu eps / sqrt|d eps . d eps|, and |d sigma| = m / (sigma |u^mu n_mu|) */
+  CCAKE_FO_DE0 = 96, CCAKE_FO_DE1, CCAKE_FO_DE2, CCAKE_FO_DE3, CCAKE_FO_N0, CCAKE_FO_N1, CCAKE_FO_N2, CCAKE_FO_N3,
+  CCAKE_FO_DSIGMA
 };
 
 /* EoS table column ids (ccake_load_eos_table): T, mu_B, mu_S, mu_Q, p, c_s^2, e, dw/ds|_n, dw/dn_B, dw/dn_S, dw/dn_Q */

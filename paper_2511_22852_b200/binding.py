@@ -23,6 +23,7 @@ MASS, WORK, NSTATE = 26, 27, 28
 SIGMA_STAR, S_DENS, RHO_B, RHO_S, RHO_Q, T, MU_B, MU_S, MU_Q = range(32, 41)
 P, E, CS2, GAMMA, NNB, CELL, THETA, SIGMA, S_STAR = range(41, 50)
 KN_PI, RE_PI, KN_BULK, RE_BULK = range(28, 32)      # applicability diagnostics, Eq. 58-61
+FO_DE0, FO_DE1, FO_DE2, FO_DE3, FO_N0, FO_N1, FO_N2, FO_N3, FO_DSIGMA = range(96, 105)   # freeze-out element, Eq. 145-148
 RHOSTAR_B, RHOSTAR_S, RHOSTAR_Q, WS, DIVV = range(50, 55)
 FM1, FM2, FM3, FK_B, FK_S, FK_Q = range(55, 61)
 RATE = 64

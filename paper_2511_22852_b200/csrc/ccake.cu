@@ -51,6 +51,8 @@ struct ccake_ctx {
   int tot_blocks = 0;
   double* arena = nullptr;      /* sorted-order doubles */
   double* diag = nullptr;       /* 4 x npad: applicability diagnostics of the latest refresh (sorted order) */
+  double* fo = nullptr;         /* 12 x npad: freeze-out element (NEXT-2): grad eps (3), d_mu eps (4), n_mu (4), |d sigma| */
+  bool fo_valid = false;
   ulonglong2* mask_cache = nullptr;   /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
   int mask_tiles = 0;
   uint32_t *cand_list = nullptr, *cand_cnt = nullptr;   /* per-block candidate lists (optional, as the mask cache) */
@@ -103,6 +105,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->tot_out); c->tot_out = nullptr;
   cudaFree(c->arena); c->arena = nullptr;
   cudaFree(c->diag); c->diag = nullptr;
+  cudaFree(c->fo); c->fo = nullptr; c->fo_valid = false;
   cudaFree(c->mask_cache); c->mask_cache = nullptr; c->mask_tiles = 0;
   cudaFree(c->cand_list); c->cand_list = nullptr; cudaFree(c->cand_cnt); c->cand_cnt = nullptr; c->cand_cap = 0;
   cudaFree(c->nnb); c->nnb = nullptr;
@@ -158,6 +161,7 @@ void carve(ccake_ctx* c) {
   s.cell_start = c->cell_start;
   s.mask_cache = c->mask_cache;
   s.mask_tiles = c->mask_tiles;
+  for (int k = 0; k < 3; ++k) s.fo_de[k] = c->fo ? c->fo + (int64_t)k * np : nullptr;
   s.cand_list = c->cand_list;
   s.cand_cnt = c->cand_cnt;
   s.cand_cap = c->cand_cap;
@@ -302,6 +306,68 @@ int rk_step(ccake_ctx* c) {
 }
 
 /* evaluate a1-a7 at the current state without an update (derived fields, rates, totals) */
+/* ---------------------------------------------------------------- NEXT-2: freeze-out surface element ---- */
+/* record of the EpsGradOp pass, sorted order: x[3], m, eps, 0, 0, 0 (reuses the smoothing-record array) */
+__global__ void fo_pack_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, Sorted so) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
+  r[0] = make_double2(so.x[0][i], so.x[1][i]);
+  r[1] = make_double2(so.x[2][i], Y[CCAKE_MASS * npad + so.perm[i]]);
+  r[2] = make_double2(so.e[i], 0.0);
+  r[3] = make_double2(0.0, 0.0);
+}
+
+/* PAPER.md Eq. 145-148 (:1466-1482) per particle, from grad eps (EpsGradOp), the rates of the latest refresh and
+   the first law: d eps/dx0 = T ds/dx0 + mu_q dn_q/dx0 along the particle with s = S sigma, n_q = N_q sigma,
+   d sigma/dx0 = -sigma theta/gamma; d_0 eps = d eps/dx0 - v^i d_i eps; n_mu = -d_mu eps / sqrt|d eps . d eps|;
+   |d sigma| = m / (sigma |u.n|).  out: 9 x npad (d_mu eps, n_mu, |d sigma|), sorted order. */
+__global__ void fo_finish_kernel(int64_t n, KParams kp, Geom gm, const double* __restrict__ Y, const double* __restrict__ K,
+                                 const double* __restrict__ theta, int64_t npad, Sorted so, double* __restrict__ out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t a = so.perm[i];
+  double u[4];
+  load_u(kp, gm, Y, npad, a, u);
+  const double gam = u[0], sig = so.sigma[i];
+  const double dsig = -sig * theta[i] / gam;
+  double deps = so.T[i] * (sig * K[CCAKE_S * npad + a] + Y[CCAKE_S * npad + a] * dsig);
+  for (int q = 0; q < NQ; ++q) deps += so.mu[q][i] * (sig * K[(CCAKE_NB + q) * npad + a] + Y[(CCAKE_NB + q) * npad + a] * dsig);
+  double de[4];
+  for (int k = 1; k <= 3; ++k) de[k] = (k <= kp.D) ? so.fo_de[k - 1][i] : 0.0;
+  de[0] = deps;
+  for (int k = 1; k <= kp.D; ++k) de[0] -= (u[k] / gam) * de[k];
+  const double gup[4] = {1.0, -1.0, -1.0, -1.0 / gm.G3};
+  double nn = 0.0;
+  for (int m = 0; m < 4; ++m) nn += gup[m] * de[m] * de[m];
+  const double norm = sqrt(fabs(nn));
+  double un = 0.0, nmu[4];
+  for (int m = 0; m < 4; ++m) { nmu[m] = (norm > 0.0) ? -de[m] / norm : 0.0; un += u[m] * nmu[m]; }
+  for (int m = 0; m < 4; ++m) { out[m * npad + i] = de[m]; out[(4 + m) * npad + i] = nmu[m]; }
+  out[8 * npad + i] = (un != 0.0) ? Y[CCAKE_MASS * npad + a] / (sig * fabs(un)) : 0.0;
+}
+
+/* runs after refresh(): one more pair pass over the same candidate lists and hit masks */
+int freezeout_pass(ccake_ctx* c) {
+  if (c->fo_valid) return CCAKE_OK;
+  const int64_t N = c->N, np = c->npad;
+  cudaStream_t st = c->stream;
+  if (!c->fo) {
+    CK(cudaMalloc(&c->fo, sizeof(double) * np * 12));
+    for (int k = 0; k < 3; ++k) c->so.fo_de[k] = c->fo + (int64_t)k * np;
+  }
+  fo_pack_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->so);
+  if (c->P.dim == 2) launch_eps_gradient<2>(N, c->kp, c->grid, c->so, st);
+  else launch_eps_gradient<3>(N, c->kp, c->grid, c->so, st);
+  fo_finish_kernel<<<nblk(N, 256), 256, 0, st>>>(N, c->kp, make_geom(c->P.coords, c->x0), c->Y[0], c->Krate, c->theta, np,
+                                                 c->so, c->fo + 3 * np);
+  c->launches += 3;
+  int rc = launch_check(c, "freezeout_pass");
+  if (rc) return rc;
+  c->fo_valid = true;
+  return CCAKE_OK;
+}
+
 int refresh(ccake_ctx* c) {
   if (c->derived_valid) return CCAKE_OK;
   if (!c->Krate) {
@@ -325,6 +391,7 @@ int refresh(ccake_ctx* c) {
   c->timing = t;
   if (rc) return rc;
   c->derived_valid = true;
+  c->fo_valid = false;
   return CCAKE_OK;
 }
 
@@ -759,6 +826,8 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
     if (c->P.eos_kind == 1 && !c->table_loaded) { c->err = "derived field before table load"; return CCAKE_ESTATE; }
     int rc = refresh(c);
     if (rc) return rc;
+    for (int k = 0; k < nfields; ++k)
+      if (ids[k] >= CCAKE_FO_DE0 && ids[k] <= CCAKE_FO_DSIGMA) { if ((rc = freezeout_pass(c))) return rc; break; }
   }
   const int64_t N = c->N, np = c->npad;
   cudaStream_t st = c->stream;
@@ -787,6 +856,10 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
       case CCAKE_CS2: src_sorted = so.cs2; break;
       case CCAKE_GAMMA: src_sorted = so.gamma; break;
       case CCAKE_THETA: src_sorted = c->theta; break;
+      case CCAKE_FO_DE0: case CCAKE_FO_DE1: case CCAKE_FO_DE2: case CCAKE_FO_DE3: case CCAKE_FO_N0: case CCAKE_FO_N1:
+      case CCAKE_FO_N2: case CCAKE_FO_N3: case CCAKE_FO_DSIGMA:
+        src_sorted = c->fo + (int64_t)(3 + id - CCAKE_FO_DE0) * np;
+        break;
       case CCAKE_KN_PI: case CCAKE_RE_PI: case CCAKE_KN_BULK: case CCAKE_RE_BULK:
         src_sorted = c->diag + (int64_t)(id - CCAKE_KN_PI) * np;
         break;

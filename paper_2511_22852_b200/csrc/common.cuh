@@ -127,6 +127,8 @@ struct Sorted {
      candidates itself); NULL / 0 = not available */
   uint32_t *cand_list, *cand_cnt;
   int cand_cap;
+  /* freeze-out element (NEXT-2): SPH gradient of eps, written by pair_kernel<EpsGradOp>; NULL until requested */
+  double* fo_de[3];
 };
 
 /* device-side status counters */

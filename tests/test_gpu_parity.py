@@ -283,3 +283,37 @@ def test_applicability_diagnostics(name):
     o.step(3)
     assert_fields(g, o, ids, 1e-8, "diagnostics after 3 steps")
     g.close()
+
+
+@pytest.mark.parametrize("name", ["C1h", "C3_small", "C4_small", "cloud2_hyp_dnmr", "cloud3_hyp_is", "cloud3_cart_closed"])
+def test_freezeout_element(name):
+    """NEXT-2 of SURVEY.md §8(f), §5.10 Eq. 145-148 (:1466-1482): d_mu eps, the outward normal n_mu and
+    |d sigma| per particle, at the loaded state and after 2 RK steps.  d_mu eps: 1e-9 of the field norm (a signed
+    SPH sum / rates); n_mu and |d sigma| are ratios of those and are compared where the gradient is not noise
+    (|d eps . d eps| above 1e-6 of its maximum): 1e-7."""
+    w = WORKLOADS[name]()
+    g, o = make_pair(w)
+    de = [B.FO_DE0, B.FO_DE1, B.FO_DE2, B.FO_DE3]
+    nn = [B.FO_N0, B.FO_N1, B.FO_N2, B.FO_N3, B.FO_DSIGMA]
+    assert tuple(de + nn) == (O.FO_DE0, O.FO_DE1, O.FO_DE2, O.FO_DE3, O.FO_N0, O.FO_N1, O.FO_N2, O.FO_N3, O.FO_DSIGMA)
+
+    def check(what, tol_de, tol_n):
+        fg, fo = g.read_fields(de + nn), o.read_fields(de + nn)
+        scale = max(float(np.max(np.abs(fo[k]))) for k in de)
+        for k in de:
+            assert np.all(np.isfinite(fg[k]))
+            assert np.max(np.abs(fg[k] - fo[k])) <= tol_de * scale, (what, k)
+        G3 = 1.0
+        inv = np.abs(fo[B.FO_DE0] ** 2 - fo[B.FO_DE1] ** 2 - fo[B.FO_DE2] ** 2 - fo[B.FO_DE3] ** 2 / G3)
+        ok = inv > 1e-6 * inv.max()
+        assert ok.sum() >= 0.05 * ok.size
+        for k in nn:
+            den = np.maximum(np.maximum(np.abs(fo[k][ok]), 1e-3 * np.max(np.abs(fo[k][ok]))), 1e-300)
+            assert np.max(np.abs(fg[k][ok] - fo[k][ok]) / den) <= tol_n, (what, k)
+
+    check("loaded state", 1e-9, 1e-7)
+    g.step(2)
+    g.synchronize()
+    o.step(2)
+    check("after 2 steps", 1e-8, 1e-6)
+    g.close()
