@@ -65,6 +65,7 @@ def lib():
         L.oracle_eos_closed_form.argtypes = [C.POINTER(Params), dbl, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_eos_forward.argtypes = [C.POINTER(Params), dbl, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_eos_table_lookup.argtypes = [vp, dbl, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32)]
+        L.oracle_smear_sources.argtypes = [vp, C.c_int64, C.POINTER(vp), C.POINTER(vp), vp, dbl, dbl, C.POINTER(vp)]
         _lib = L
     return _lib
 
@@ -157,6 +158,18 @@ class Oracle:
         self._chk(lib().oracle_read_neighbors(self._h, counts.ctypes.data, offsets.ctypes.data, lst.ctypes.data,
                                               lst.size), "oracle_read_neighbors")
         return counts, offsets, lst
+
+    def smear_sources(self, p, r, t, h_source, eta_norm=1.0):
+        """oracle_smear_sources (Eq. 35): p [4, np], r [3, np], t [np] -> j [4, n]."""
+        p = np.ascontiguousarray(p, dtype=np.float64); r = np.ascontiguousarray(r, dtype=np.float64)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        out = np.zeros((4, self.n), dtype=np.float64)
+        pp = (C.c_void_p * 4)(*[p[m].ctypes.data for m in range(4)])
+        rr = (C.c_void_p * 3)(*[r[a].ctypes.data for a in range(3)])
+        oo = (C.c_void_p * 4)(*[out[m].ctypes.data for m in range(4)])
+        self._chk(lib().oracle_smear_sources(self._h, t.size, pp, rr, t.ctypes.data, float(h_source), float(eta_norm), oo),
+                  "oracle_smear_sources")
+        return out
 
     def eos_table_lookup(self, s, n):
         out = (C.c_double * 11)()

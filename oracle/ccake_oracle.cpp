@@ -1334,4 +1334,26 @@ int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double o
   return ORACLE_OK;
 }
 
+int oracle_smear_sources(oracle_ctx* c, int64_t np, const double* const p[4], const double* const r[3], const double* t,
+                         double h_source, double eta_norm, double* const j[4]) {
+  if (!c || np < 0 || !p || !r || !t || !j || !(h_source > 0.0)) return ORACLE_EINVAL;
+  if (!c->loaded) return ORACLE_ESTATE;
+  const int D = c->P.dim;
+  const Geometry g = geometry(c->P, c->x0);
+  const double x0 = c->x0, dx0 = c->P.dx0;
+  const double pref = eta_norm / (dx0 * g.sqrtg);
+  for (int64_t i = 0; i < c->N; ++i) {
+    double acc[4] = {0, 0, 0, 0};
+    for (int64_t k = 0; k < np; ++k) {
+      if (!(t[k] > x0 - dx0 && t[k] <= x0)) continue;            /* Eq. 35: x0 - dx0 < t_k <= x0 */
+      double r2 = 0.0;
+      for (int a = 0; a < D; ++a) { const double dr = c->y.f[OF_R1 + a][i] - r[a][k]; r2 += dr * dr; }
+      const double W = kernel_W(D, h_source, std::sqrt(r2));
+      for (int m = 0; m < 4; ++m) acc[m] += p[m][k] * W;
+    }
+    for (int m = 0; m < 4; ++m) j[m][i] = pref * acc[m];
+  }
+  return ORACLE_OK;
+}
+
 }  /* extern "C" */

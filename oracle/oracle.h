@@ -86,6 +86,14 @@ int oracle_eos_closed_form(const oracle_params* p, double s, const double n[3], 
 int oracle_eos_forward(const oracle_params* p, double T, const double mu[3], double out[5]);
 int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double out[11], int32_t* oob);
 
+/* Source smearing of PAPER.md Eq. 35 (:521), the gather half of the dynamical initialisation: for every loaded
+ * particle i,  j^mu_i = eta_norm / (dx0 sqrt(-g)) * sum over partons k with x0 - dx0 < t_k <= x0 of
+ * p^mu_k W(r_i - r_k; h_source), W the cubic spline of Eq. 77 in the context's dimension, x0 the current time and
+ * dx0 the step of the context.  p: 4 columns, r: 3 columns (dim used), t: formation times, np entries each;
+ * j: 4 columns of n doubles (particle order).  The state is not modified. */
+int oracle_smear_sources(oracle_ctx* c, int64_t np, const double* const p[4], const double* const r[3], const double* t,
+                         double h_source, double eta_norm, double* const j[4]);
+
 #ifdef __cplusplus
 }
 #endif

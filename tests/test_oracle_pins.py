@@ -779,3 +779,45 @@ def test_freezeout_normal_on_gubser():
         assert abs(f[O.FO_DSIGMA] * f[O.SIGMA] * abs(un) - 1) < (0.25 if h > 0.2 else 0.07)
     assert errs[0][0] < 0.12 and errs[0][1] < 0.12 and errs[1][0] < 0.03 and errs[1][1] < 0.03
     assert errs[0][0] / errs[1][0] > 3.0 and errs[0][1] / errs[1][1] > 3.0
+
+
+def _source_setup(D, coords, n, dx, tau0=1.3, dt=0.1):
+    x1 = (np.arange(n) - 0.5 * (n - 1)) * dx
+    grids = np.meshgrid(*([x1] * D), indexing="ij")
+    p = W.base_params(dim=D, coords=coords, eom=0, eos_kind=0, h=0.3, x0_start=tau0, dx0=dt)
+    o = O.Oracle(**p)
+    f = {O.R1 + k: grids[k].ravel() for k in range(D)}
+    f[O.S] = np.full(grids[0].size, 1.0)
+    o.load_particles(f)
+    return o, [g.ravel() for g in grids], tau0, dt
+
+
+@pytest.mark.parametrize("D,coords", [(2, 0), (2, 1), (3, 1)])
+def test_source_smearing_closed_forms(D, coords):
+    """PAPER.md Eq. 35 (:521).  (1) One parton sitting on a particle: j^mu there = eta p^mu sigma_D(h_s) / (dx0 sqrt(-g))
+    with sigma_2 = 10/(7 pi h^2), sigma_3 = 1/(pi h^3) (Eq. 77) and sqrt(-g) = tau or 1; at distance >= 2 h_s: 0.
+    (2) Partition of unity on the lattice (h_s = 1.4 fm >> dx): sum_i j^mu_i dV = eta sum_k p^mu_k / (dx0 sqrt(-g)) over the
+    partons inside the time window, to 2e-6 of sum |p|.  (3) The window is x0 - dx0 < t_k <= x0 exactly.  (4) Linear in p."""
+    n, dx, hs, eta = (41, 0.2, 1.4, 0.62) if D == 2 else (21, 0.4, 1.4, 0.62)
+    o, xs, tau0, dt = _source_setup(D, coords, n, dx)
+    sqrtg = tau0 if coords == 1 else 1.0
+    ic = int(np.argmin(sum(x * x for x in xs)))
+    r0 = [xs[k][ic] for k in range(D)] + [0.0] * (3 - D)
+    p1 = np.array([[2.0], [0.3], [-0.4], [0.1]])
+    j = o.smear_sources(p1, np.array(r0)[:, None], [tau0], hs, eta)
+    sig = 10.0 / (7.0 * np.pi * hs * hs) if D == 2 else 1.0 / (np.pi * hs ** 3)
+    assert np.allclose(j[:, ic], eta * p1[:, 0] * sig / (dt * sqrtg), rtol=1e-13)
+    dist = np.sqrt(sum((xs[k] - r0[k]) ** 2 for k in range(D)))
+    assert np.all(j[:, dist >= 2 * hs] == 0.0) and np.all(j[0, dist < 2 * hs - 1e-9] > 0.0)
+    # (2) + (3): five partons near the centre, two of them outside the time window
+    rng = np.random.default_rng(35)
+    rp = np.zeros((3, 5)); rp[:D] = rng.uniform(-0.6, 0.6, (D, 5))
+    pp = rng.normal(0, 1, (4, 5)); pp[0] = np.abs(pp[0]) + 1
+    tt = np.array([tau0, tau0 - 0.5 * dt, tau0 - dt + 1e-12, tau0 - dt, tau0 + 1e-12])     # last two: outside
+    j = o.smear_sources(pp, rp, tt, hs, eta)
+    tot = j.sum(axis=1) * dx ** D
+    ref = eta * pp[:, :3].sum(axis=1) / (dt * sqrtg)
+    assert np.max(np.abs(tot - ref)) <= 2e-6 * eta * np.abs(pp[:, :3]).sum() / (dt * sqrtg)
+    # (4)
+    j2 = o.smear_sources(2.5 * pp, rp, tt, hs, eta)
+    assert np.max(np.abs(j2 - 2.5 * j)) <= 1e-13 * np.max(np.abs(j2))
