@@ -132,6 +132,17 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
                            int32_t memspace);
 
 /* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
+/* NEXT-3 (part) of SURVEY.md §8(f): the source smearing of PAPER.md Eq. 35 (:521), the gather half of the dynamical
+ * initialisation.  For every loaded particle i, at the context's current time x0 and step dx0,
+ *   j^mu_i = eta_norm / (dx0 sqrt(-g)) * sum over partons k with x0 - dx0 < t[k] <= x0 of p[mu][k] W(r_i - r[.][k]; h_source),
+ * W the cubic spline of Eq. 77 in the context's dimension (2 h_source cut-off), sqrt(-g) = tau (hyperbolic) or 1.
+ * p: 4 columns, r: 3 columns (the first `dim` are used), t: formation times — npartons doubles each; j: 4 columns of
+ * n doubles in the caller's particle order; all in `memspace`.  Every parton is tested against every particle (no
+ * spatial index: parton counts per step are thousands).  The state is not modified: feeding j^mu into the equations
+ * of motion (I^nu, I_q) is not built. */
+int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
+                        const double* t, double h_source, double eta_norm, double* const j[4], int32_t memspace);
+
 int ccake_step(ccake_ctx* c, int32_t nsteps);
 
 /* Wait for the stream.  ERANGE when, since the last load, a particle left the EoS table, a per-particle solve

@@ -14,6 +14,7 @@
  *   Step 6  integrator                    not in the paper (DESIGN reading 7): RK2 midpoint / classical RK4
  *   Step 7  conserved totals              §5.6.5 :1049-1063
  *   extra   applicability diagnostics     Eq. 58-61 :797-805 (Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1; pinned on Bjorken)
+ *   extra   source smearing               Eq. 35 :521 (pinned: single parton, partition of unity, window, linearity)
  *   extra   freeze-out surface element    Eq. 145-148 :1466-1482 (d_mu eps, n_mu, |d sigma|; pinned on Bjorken, Gubser)
  *
  * There is no blocking, fusion or reordering: loops are gather form (for a { for b }), the per-particle linear

@@ -30,7 +30,7 @@ RATE = 64
 HOST, DEVICE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table",
+EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_smear_sources",
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
@@ -74,6 +74,7 @@ def lib():
         L.ccake_load_particles.argtypes = [vp, i64, i32, C.POINTER(i32), C.POINTER(vp), i32]
         L.ccake_load_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
         L.ccake_invert_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
+        L.ccake_smear_sources.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp), i32]
         L.ccake_step.argtypes = [vp, i32]
         L.ccake_synchronize.argtypes = [vp]
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
@@ -186,6 +187,18 @@ class Ccake:
         self._chk(lib().ccake_invert_eos_table(self._h, dims, kinds, ptrs, len(col_ids), cids,
                                                res.ctypes.data if out else None, HOST), "ccake_invert_eos_table")
         return res
+
+    def smear_sources(self, p, r, t, h_source, eta_norm=1.0):
+        """ccake_smear_sources (Eq. 35): p [4, np], r [3, np], t [np] (numpy, host) -> j [4, n] numpy."""
+        p = np.ascontiguousarray(p, dtype=np.float64); r = np.ascontiguousarray(r, dtype=np.float64)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        out = np.zeros((4, self.n), dtype=np.float64)
+        pp = (C.c_void_p * 4)(*[p[m].ctypes.data for m in range(4)])
+        rr = (C.c_void_p * 3)(*[r[a].ctypes.data for a in range(3)])
+        oo = (C.c_void_p * 4)(*[out[m].ctypes.data for m in range(4)])
+        self._chk(lib().ccake_smear_sources(self._h, t.size, pp, rr, t.ctypes.data, float(h_source), float(eta_norm),
+                                            oo, HOST), "ccake_smear_sources")
+        return out
 
     def step(self, nsteps=1):
         self._chk(lib().ccake_step(self._h, nsteps), "ccake_step")

@@ -368,6 +368,51 @@ int freezeout_pass(ccake_ctx* c) {
   return CCAKE_OK;
 }
 
+/* ------------------------------------------------------------------ NEXT-3 (part): source smearing ---- */
+/* PAPER.md Eq. 35 (:521).  One thread per particle (store order); the partons stream through shared memory in
+   tiles of SRC_TILE (position, four-momentum; a parton outside the time window is staged with zero momentum and a
+   position that fails the cut-off test).  src: 8 x np doubles (p0..p3, r0..r2, t). */
+constexpr int SRC_TILE = 128;
+template <int D>
+__global__ void __launch_bounds__(SRC_TILE)
+smear_sources_kernel(int64_t n, int64_t npad, const double* __restrict__ Y, const uint32_t* __restrict__ orig, int64_t np_,
+                     const double* __restrict__ src, double x0, double dx0, double pref, double hs, double sig_d,
+                     double* __restrict__ out) {
+  __shared__ double sp[4][SRC_TILE], sr[3][SRC_TILE];
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  const int64_t ic = (i < n) ? i : n - 1;
+  double xa[3] = {0.0, 0.0, 0.0};
+  for (int k = 0; k < D; ++k) xa[k] = Y[(CCAKE_R1 + k) * npad + ic];
+  const double inv_h = 1.0 / hs, cut2 = (2.0 * hs) * (2.0 * hs);
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int64_t base = 0; base < np_; base += SRC_TILE) {
+    const int64_t k = base + threadIdx.x;
+    __syncthreads();
+    {
+      const bool in = k < np_ && src[7 * np_ + k] > x0 - dx0 && src[7 * np_ + k] <= x0;       /* x0 - dx0 < t_k <= x0 */
+      for (int m = 0; m < 4; ++m) sp[m][threadIdx.x] = in ? src[m * np_ + k] : 0.0;
+      for (int a = 0; a < 3; ++a) sr[a][threadIdx.x] = in ? src[(4 + a) * np_ + k] : 1.0e150;
+    }
+    __syncthreads();
+    const int cnt = (int)min((int64_t)SRC_TILE, np_ - base);
+    for (int b = 0; b < cnt; ++b) {
+      double r2 = 0.0;
+#pragma unroll
+      for (int a = 0; a < D; ++a) { const double dr = xa[a] - sr[a][b]; r2 += dr * dr; }
+      if (r2 < cut2) {
+        const double q = sqrt(r2) * inv_h, t = 2.0 - q;
+        const double W = sig_d * ((q <= 1.0) ? fma(q * q, fma(0.75, q, -1.5), 1.0) : 0.25 * t * t * t);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) acc[m] = fma(sp[m][b], W, acc[m]);
+      }
+    }
+  }
+  if (i < n) {
+    const int64_t o = orig[i];
+    for (int m = 0; m < 4; ++m) out[m * n + o] = pref * acc[m];
+  }
+}
+
 int refresh(ccake_ctx* c) {
   if (c->derived_valid) return CCAKE_OK;
   if (!c->Krate) {
@@ -784,6 +829,48 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
     }
   cudaFree(dax);
   cudaFree(ddata);
+  return rc;
+}
+
+int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3], const double* t,
+                        double h_source, double eta_norm, double* const j[4], int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (npartons < 0 || !p || !r || !t || !j || !(h_source > 0.0) || (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_smear_sources";
+    return CCAKE_EINVAL;
+  }
+  for (int m = 0; m < 4; ++m) if (!p[m] || !j[m]) { c->err = "null column"; return CCAKE_EINVAL; }
+  for (int a = 0; a < 3; ++a) if (!r[a]) { c->err = "null column"; return CCAKE_EINVAL; }
+  if (!c->loaded) { c->err = "smear before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  const int64_t N = c->N, np = c->npad, ns = npartons;
+  cudaStream_t st = c->stream;
+  const cudaMemcpyKind in = (memspace == CCAKE_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const cudaMemcpyKind outk = (memspace == CCAKE_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+  double *dsrc = nullptr, *dout = nullptr;
+  CK(cudaMalloc(&dsrc, sizeof(double) * 8 * std::max<int64_t>(ns, 1)));
+  if (cudaMalloc(&dout, sizeof(double) * 4 * N) != cudaSuccess) { cudaFree(dsrc); c->err = "source buffers"; return CCAKE_ENOMEM; }
+  for (int m = 0; m < 4 && ns > 0; ++m) cudaMemcpyAsync(dsrc + m * ns, p[m], sizeof(double) * ns, in, st);
+  for (int a = 0; a < 3 && ns > 0; ++a) cudaMemcpyAsync(dsrc + (4 + a) * ns, r[a], sizeof(double) * ns, in, st);
+  if (ns > 0) cudaMemcpyAsync(dsrc + 7 * ns, t, sizeof(double) * ns, in, st);
+  const Geom gm = make_geom(c->P.coords, c->x0);
+  const double pi = 3.14159265358979323846;
+  const int D = c->P.dim;
+  const double sig_d = (D == 2) ? 10.0 / (7.0 * pi * h_source * h_source) : 1.0 / (pi * h_source * h_source * h_source);
+  const double pref = eta_norm / (c->P.dx0 * gm.sqrtg);
+  if (D == 2)
+    smear_sources_kernel<2><<<nblk(N, SRC_TILE), SRC_TILE, 0, st>>>(N, np, c->Y[0], c->orig[0], ns, dsrc, c->x0, c->P.dx0, pref,
+                                                                   h_source, sig_d, dout);
+  else
+    smear_sources_kernel<3><<<nblk(N, SRC_TILE), SRC_TILE, 0, st>>>(N, np, c->Y[0], c->orig[0], ns, dsrc, c->x0, c->P.dx0, pref,
+                                                                   h_source, sig_d, dout);
+  c->launches += 1;
+  int rc = launch_check(c, "smear_sources_kernel");
+  for (int m = 0; m < 4 && rc == CCAKE_OK; ++m)
+    if (cudaMemcpyAsync(j[m], dout + m * N, sizeof(double) * N, outk, st) != cudaSuccess) { c->err = "copy of j"; rc = CCAKE_ECUDA; }
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == CCAKE_OK) { c->err = "smear_sources failed"; rc = CCAKE_ECUDA; }
+  cudaFree(dsrc);
+  cudaFree(dout);
   return rc;
 }
 
