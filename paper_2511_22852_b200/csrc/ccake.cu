@@ -15,7 +15,7 @@
 #include "common.cuh"
 #include "eom.cuh"
 #include "grid_sort.cuh"
-#include "pair_tiled.cuh"
+#include "pair_mma.cuh"
 #include "thermo_eos.cuh"
 #include "totals.cuh"
 
@@ -53,7 +53,7 @@ struct ccake_ctx {
   double* diag = nullptr;       /* 4 x npad: applicability diagnostics of the latest refresh (sorted order) */
   double* fo = nullptr;         /* 12 x npad: freeze-out element (NEXT-2): grad eps (3), d_mu eps (4), n_mu (4), |d sigma| */
   bool fo_valid = false;
-  ulonglong2* mask_cache = nullptr;   /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
+  uint4* mask_cache = nullptr;        /* hit masks of the smoothing pass (optional: absent if the allocation fails) */
   int mask_tiles = 0;
   uint32_t *cand_list = nullptr, *cand_cnt = nullptr;   /* per-block candidate lists (optional, as the mask cache) */
   int cand_cap = 0;
@@ -307,14 +307,15 @@ int rk_step(ccake_ctx* c) {
 
 /* evaluate a1-a7 at the current state without an update (derived fields, rates, totals) */
 /* ---------------------------------------------------------------- NEXT-2: freeze-out surface element ---- */
-/* record of the EpsGradOp pass, sorted order: x[3], m, eps, 0, 0, 0 (reuses the smoothing-record array) */
+/* record of the EpsGradOp pass, sorted order: x[3], m, m eps, 0, 0, 0 (reuses the smoothing-record array) */
 __global__ void fo_pack_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, Sorted so) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
   r[0] = make_double2(so.x[0][i], so.x[1][i]);
-  r[1] = make_double2(so.x[2][i], Y[CCAKE_MASS * npad + so.perm[i]]);
-  r[2] = make_double2(so.e[i], 0.0);
+  const double m = Y[CCAKE_MASS * npad + so.perm[i]];
+  r[1] = make_double2(so.x[2][i], m);
+  r[2] = make_double2(m * so.e[i], 0.0);
   r[3] = make_double2(0.0, 0.0);
 }
 
@@ -654,20 +655,24 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   CK(cudaMalloc(&c->arena, sizeof(double) * np * ARENA_FIELDS));
   CK(cudaMemsetAsync(c->arena, 0, sizeof(double) * np * ARENA_FIELDS, c->stream));
   {
-    /* hit-mask cache: MASK_TILES tiles per pair block, 16 B per stream and tile; capped at 1/8 of the free memory
-       and dropped altogether if the allocation fails — the gradient pass then computes its masks itself */
-    const size_t nblocks = (size_t)((c->N + BH - 1) / BH), per_tile = sizeof(ulonglong2) * (PT / CCAKE_PAIR_LPS);
+    /* hit-mask cache: MASK_TILES tiles per pair block, 16 B per group of 8 homes and tile; capped at 1/8 of the free
+       memory and dropped altogether if the allocation fails — the gradient pass then culls for itself.  Test knobs
+       (include/ccake.h): the environment variables CCAKE_MASK_TILES and CCAKE_CAND_CAP override the two sizes. */
+    const size_t nblocks = (size_t)((c->N + BH - 1) / BH), per_tile = sizeof(uint4) * NGRP;
     size_t free_b = 0, total_b = 0;
     int tiles = MASK_TILES;
+    if (const char* e = std::getenv("CCAKE_MASK_TILES")) tiles = std::max(0, std::atoi(e));
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess)
       while (tiles > 0 && nblocks * tiles * per_tile > free_b / 8) tiles /= 2;
     if (tiles > 0 && cudaMalloc(&c->mask_cache, nblocks * tiles * per_tile) == cudaSuccess) c->mask_tiles = tiles;
     else { cudaGetLastError(); c->mask_cache = nullptr; c->mask_tiles = 0; }
-    /* candidate lists: CAND_CAP entries per pair block, same policy */
-    int cap = CAND_CAP;
+    /* candidate lists: CAND_CAP entries per pair block, same policy; a block whose candidates do not fit lists them
+       inside the pass */
+    int cap = CAND_CAP, cap_min = 2048;
+    if (const char* e = std::getenv("CCAKE_CAND_CAP")) { cap = std::max(0, std::atoi(e)); cap_min = 1; }
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess)
-      while (cap >= 2048 && nblocks * cap * sizeof(uint32_t) > free_b / 8) cap /= 2;
-    if (cap >= 2048 && cudaMalloc(&c->cand_list, nblocks * cap * sizeof(uint32_t)) == cudaSuccess &&
+      while (cap >= cap_min && cap > 0 && nblocks * cap * sizeof(uint32_t) > free_b / 8) cap /= 2;
+    if (cap >= cap_min && cap > 0 && cudaMalloc(&c->cand_list, nblocks * cap * sizeof(uint32_t)) == cudaSuccess &&
         cudaMalloc(&c->cand_cnt, nblocks * sizeof(uint32_t)) == cudaSuccess) c->cand_cap = cap;
     else { cudaGetLastError(); cudaFree(c->cand_list); cudaFree(c->cand_cnt); c->cand_list = c->cand_cnt = nullptr; c->cand_cap = 0; }
   }
@@ -1061,8 +1066,10 @@ int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity) {
   const int64_t N = c->N;
   unsigned long long* d = nullptr;
   CK(cudaMalloc(&d, sizeof(unsigned long long) * N));
-  if (c->P.dim == 2) neighbour_walk_kernel<2><<<nblk(N, 128), 128, 0, c->stream>>>(N, c->kp, c->grid, c->so, c->orig[0], 0, d, nullptr, nullptr);
-  else neighbour_walk_kernel<3><<<nblk(N, 128), 128, 0, c->stream>>>(N, c->kp, c->grid, c->so, c->orig[0], 0, d, nullptr, nullptr);
+  /* the smoothing pass itself, in its hashing instantiation: the sets hashed are the ones pair_mma_kernel used */
+  if (c->P.dim == 2) launch_smoothing_hash<2>(N, c->kp, c->grid, c->so, c->orig[0], d, c->stream);
+  else launch_smoothing_hash<3>(N, c->kp, c->grid, c->so, c->orig[0], d, c->stream);
+  c->launches += 1;
   cudaError_t e = cudaMemcpyAsync(out, d, sizeof(unsigned long long) * N, cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   cudaFree(d);

@@ -115,12 +115,12 @@ struct Sorted {
   /* a5 */
   double *gamma, *sigma, *s, *n[NQ];
   double *T, *mu[NQ], *p, *e, *cs2, *ws, *wq[NQ];
-  double* rec_g;      /* [n][NREC]: AoS payload of the gradient pass, layout GLayout (pair_tiled.cuh) */
+  double* rec_g;      /* [n][NREC]: AoS payload of the gradient pass, layout GLayout (pair_mma.cuh) */
   /* a6 */
   double *FP[3], *FB[3], *FK[NQ], *DU[9], *DA[9], *divv;
-  /* hit masks of the smoothing pass, reused by the gradient pass of the same substep (pair_tiled.cuh):
-     [pair block][tile number < mask_tiles][stream] x 128 bit; NULL / 0 = no reuse */
-  ulonglong2* mask_cache;
+  /* hit masks of the smoothing pass, reused by the gradient pass of the same substep (pair_mma.cuh):
+     [pair block][tile number < mask_tiles][group of 8 homes] x 128 bit; NULL / 0 = no reuse */
+  uint4* mask_cache;
   int mask_tiles;
   /* candidate lists of the pair blocks, written once per substep by cand_list_kernel and read by both passes:
      block b owns cand_list[b * cand_cap ...], cand_cnt[b] entries (0xffffffff: did not fit, the pass lists its

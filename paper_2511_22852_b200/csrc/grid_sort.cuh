@@ -350,12 +350,14 @@ __global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad
   const uint32_t a = perm[i];
   const double x = Y[CCAKE_R1 * npad + a], y = Y[CCAKE_R2 * npad + a], z = (D == 3) ? Y[CCAKE_R3 * npad + a] : 0.0;
   so.x[0][i] = x; so.x[1][i] = y; so.x[2][i] = z;
-  so.xf[i] = make_float4((float)(x - grid->xmin[0]), (float)(y - grid->xmin[1]), (D == 3) ? (float)(z - grid->xmin[2]) : 0.f, 0.f);
+  so.xf[i] = make_float4((float)(x - grid->xmin[0]), (float)(y - grid->xmin[1]), (D == 3) ? (float)(z - grid->xmin[2]) : 0.f,
+                         __uint_as_float((uint32_t)i));   /* w: the sorted slot (read by the neighbour-hash test pass) */
   double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
   r[0] = make_double2(x, y);
-  r[1] = make_double2(z, Y[CCAKE_MASS * npad + a]);
-  r[2] = make_double2(Y[CCAKE_S * npad + a], Y[CCAKE_NB * npad + a]);
-  r[3] = make_double2(Y[CCAKE_NS * npad + a], Y[CCAKE_NQ * npad + a]);
+  const double m = Y[CCAKE_MASS * npad + a];              /* payload columns carry the SPH weight m_b (pair_mma.cuh) */
+  r[1] = make_double2(z, m);
+  r[2] = make_double2(m * Y[CCAKE_S * npad + a], m * Y[CCAKE_NB * npad + a]);
+  r[3] = make_double2(m * Y[CCAKE_NS * npad + a], m * Y[CCAKE_NQ * npad + a]);
 }
 
 }  // namespace ccake

@@ -8,7 +8,7 @@
  */
 #pragma once
 #include "common.cuh"
-#include "pair_tiled.cuh"
+#include "pair_mma.cuh"
 
 namespace ccake {
 
@@ -255,25 +255,27 @@ thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restr
   else load_dissip<2>(kp, gm, Y, npad, a, u, ds);
   const double sst2 = sst * sst;
   const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
-  /* AoS payload record of the gradient pass (layout GLayout): x[D], m, P, u[D], v[D], B[D*D], K[3*D], alpha[3] */
+  /* AoS payload record of the gradient pass (layout GLayout): x[D], m, then m times each of P, u[D], v[D], B[D*D],
+     K[3*D], alpha[3] — the pair pass multiplies a column of b by the pair weight without m_b (pair_mma.cuh) */
   const GLayout L = make_glayout(D, kp.shear != 0, kp.diff != 0);
   double* __restrict__ rg = so.rec_g + i * L.NREC;
+  const double mb = Y[CCAKE_MASS * npad + a];
   for (int k = 0; k < D; ++k) rg[k] = so.x[k][i];
-  rg[L.M] = Y[CCAKE_MASS * npad + a];
-  rg[L.P] = (th.p + ds.bulkt * sig) / sst2;
-  for (int j = 1; j <= D; ++j) { rg[L.U + j - 1] = u[j]; rg[L.V + j - 1] = u[j] / gam; }
+  rg[L.M] = mb;
+  rg[L.P] = mb * ((th.p + ds.bulkt * sig) / sst2);
+  for (int j = 1; j <= D; ++j) { rg[L.U + j - 1] = mb * u[j]; rg[L.V + j - 1] = mb * (u[j] / gam); }
   if (kp.shear)
     for (int j = 1; j <= D; ++j)
       for (int k = 1; k <= D; ++k) {
         const double pi_j_k = sig * ds.pit[j][k] * glo[k];
         const double pi_0_k = sig * ds.pit[0][k] * glo[k];
-        rg[L.B + (j - 1) * D + (k - 1)] = (pi_j_k - (u[j] / gam) * pi_0_k) / sst2;
+        rg[L.B + (j - 1) * D + (k - 1)] = mb * ((pi_j_k - (u[j] / gam) * pi_0_k) / sst2);
       }
   if (kp.diff) {
     for (int q = 0; q < NQ; ++q) {
-      rg[L.AL + q] = th.mu[q] / th.T;
+      rg[L.AL + q] = mb * (th.mu[q] / th.T);
       for (int j = 1; j <= D; ++j)
-        rg[L.K + q * D + (j - 1)] = (sig * ds.Jt[q][j] - (u[j] / gam) * sig * ds.Jt[q][0]) / sst2;
+        rg[L.K + q * D + (j - 1)] = mb * ((sig * ds.Jt[q][j] - (u[j] / gam) * sig * ds.Jt[q][0]) / sst2);
     }
   }
   for (int k = L.AL + (kp.diff ? 3 : 0); k < L.NREC; ++k) rg[k] = 0.0;
