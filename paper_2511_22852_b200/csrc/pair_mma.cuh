@@ -322,8 +322,9 @@ template <class Op> struct PairCfg {
   static constexpr size_t B_PAY = sizeof(double2) * NU * CSTRIDE;
   static constexpr size_t B_PAYX = sizeof(float4) * TILE_B;
   static constexpr size_t B_LIST = sizeof(uint32_t) * (LCAP + LB * PT);
-  static constexpr size_t B_FIFO = NGRP * HALF_B;           /* tile slots waiting per group */
-  static constexpr size_t B_RING = B_PAY + B_PAYX + B_LIST + B_FIFO;
+  static constexpr size_t B_FIFO = sizeof(uint16_t) * NGRP * HALF_B;   /* tile entries waiting per group */
+  static constexpr size_t B_MASK = sizeof(uint4) * NSLOT * NGRP;
+  static constexpr size_t B_RING = B_PAY + B_PAYX + B_LIST + B_FIFO + B_MASK;
   static constexpr size_t B_SCRATCH = sizeof(double) * BH * SSTRIDE;
   static constexpr size_t SMEM = (B_RING > B_SCRATCH) ? B_RING : B_SCRATCH;
 };
@@ -432,6 +433,11 @@ cand_list_kernel(int64_t n, const Grid* __restrict__ grid, Sorted so) {
   if (tid == 0) so.cand_cnt[blockIdx.x] = (nrel <= cap) ? nrel : 0xffffffffu;
 }
 
+#ifdef CCAKE_PAIR_PROF
+/* experiment builds only: [0] quads of all warps, [1] sum over blocks of (warps x max quads of a warp), per pass kind */
+__device__ unsigned long long g_pair_prof[16];
+#endif
+
 __device__ __forceinline__ uint64_t pm_mix64(uint64_t z) {      /* splitmix64 finaliser (include/ccake.h) */
   z += 0x9E3779B97F4A7C15ULL;
   z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
@@ -455,7 +461,8 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   double2* pay = reinterpret_cast<double2*>(smem_raw);                  /* [NU][CSTRIDE] staged records        */
   float4* payx = reinterpret_cast<float4*>(pay + NU * CSTRIDE);         /* [TILE_B] FP32 positions of the tile */
   uint32_t* list = reinterpret_cast<uint32_t*>(payx + TILE_B);          /* [LCAP + LB * PT] block candidate list */
-  uint8_t* fifo = reinterpret_cast<uint8_t*>(list + LCAP + LB * PT);    /* [NGRP][HALF_B] tile entries that passed, per group */
+  uint16_t* fifo = reinterpret_cast<uint16_t*>(list + LCAP + LB * PT);  /* [NGRP][HALF_B] byte offsets of the staged entries that passed, per group */
+  uint4* mstage = reinterpret_cast<uint4*>(fifo + NGRP * HALF_B);       /* [NSLOT][NGRP] cached hit masks of the staged tiles (MC == 2) */
   __shared__ float s_lo[NW][3], s_hi[NW][3];
   __shared__ int wcnt[LB * NW];
   __shared__ uint32_t rb0[MAXROW], rcum[MAXROW + 1];
@@ -540,12 +547,15 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
 #pragma unroll
   for (int gg = 0; gg < GPW; ++gg) { hits[gg] = 0u; hsum[gg] = 0ull; }
   int nrel = 0;
+#ifdef CCAKE_PAIR_PROF
+  unsigned prof_quads = 0;
+#endif
 
   /* one quad: lane (gid, tig) evaluates the pair (home gid of the group, candidate tig of the quad) and the warp
-     accumulates 8 homes x 4 candidates x 8 columns per MMA.  kb: slot of the lane's candidate in the ring.  Returns
+     accumulates 8 homes x 4 candidates x 8 columns per MMA.  koff: byte offset of the lane's candidate in the ring.  Returns
      (smoothing pass) the 4 bits "candidate t of the quad is within 2h of at least one home of the group". */
-  auto quad = [&](const int gg, const uint32_t kb, const bool act) -> uint32_t {
-    const double2* __restrict__ p = pay + kb;
+  auto quad = [&](const int gg, const uint32_t koff, const bool act) -> uint32_t {
+    const double2* __restrict__ p = reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(pay) + koff);
     const double2 h0 = p[0];
     const double zb = (D == 3) ? reinterpret_cast<const double*>(p + CSTRIDE)[0] : 0.0;
     PairGeom<D> pg;
@@ -559,7 +569,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
       for (int j = 0; j < NJ; ++j) bop[T][j] = *reinterpret_cast<const double*>(rb + boff[T][j]);
     if (Op::COUNT) hits[gg] += pg.hit ? 1u : 0u;
     if (Op::HASH) {
-      const uint32_t slot = __float_as_uint(payx[kb].w);       /* sorted slot of the candidate (pack_smoothing_kernel) */
+      const uint32_t slot = __float_as_uint(payx[koff >> 4].w);  /* sorted slot of the candidate (pack_smoothing_kernel) */
       if (pg.hit && (int64_t)slot != ih[gg]) hsum[gg] += pm_mix64((uint64_t)orig[so.perm[slot]] + 1ULL);
     }
     uint32_t nib = 0u;
@@ -576,12 +586,6 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   /* hit-mask cache: [block][tile][group] x 128 bit */
   const int mtiles = (MC != 0 && so.mask_cache != nullptr) ? so.mask_tiles : 0;
   uint4* __restrict__ mrow = reinterpret_cast<uint4*>(so.mask_cache) + (size_t)blockIdx.x * (size_t)max(mtiles, 1) * NGRP;
-  uint4 mnext[GPW];
-#pragma unroll
-  for (int gg = 0; gg < GPW; ++gg) {
-    mnext[gg] = make_uint4(0u, 0u, 0u, 0u);
-    if (MC == 2 && mtiles > 0) mnext[gg] = __ldg(mrow + (w * GPW + gg));
-  }
   /* the candidates come from the global list of this block (cand_list_kernel) or, if that is absent or did not
      fit, from the list in shared memory filled further below */
   const uint32_t gcnt = (so.cand_cap > 0) ? so.cand_cnt[blockIdx.x] : 0xffffffffu;
@@ -598,10 +602,14 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
     }
     return j;
   };
-  auto issue = [&](const uint32_t j, const int slot, const bool need_x) {
+  const uint32_t mstage_s = (uint32_t)__cvta_generic_to_shared(mstage);
+  auto issue = [&](const uint32_t j, const int slot, const bool need_x, const int u) {
     /* warp w copies entries [w * RPW, (w + 1) * RPW) of the tile: FP32 position (a 16-byte copy by the owning lane) and
        the records unit by unit, consecutive lanes taking consecutive units (coalesced rows) */
     const int sb = slot * HALF_B;
+    if (MC == 2 && !need_x && lane < GPW)           /* the cached hit masks of the warp's groups travel with the tile */
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(mstage_s + (uint32_t)(slot * NGRP + w * GPW + lane) * 16u),
+                   "l"(mrow + (size_t)u * NGRP + (w * GPW + lane)));
     if (need_x && j != 0xffffffffu)                 /* padding entries keep stale data; the masks leave them out */
       asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(payx_s + (uint32_t)(sb + w * RPW + lane) * 16u), "l"(xf + j));
 #pragma unroll
@@ -639,9 +647,9 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
         const int u = tt0 + ni;
         if (!all_done(u - NSLOT)) {
           if (!block) break;
-          do { __nanosleep(256); } while (!all_done(u - NSLOT));
+          do { __nanosleep(1000); } while (!all_done(u - NSLOT));
         }
-        issue(jn, u % NSLOT, MC != 2 || u >= mtiles);
+        issue(jn, u % NSLOT, MC != 2 || u >= mtiles, u);
         ++ni;
         jn = load_j(cnt, ntile, ni);
       }
@@ -656,21 +664,22 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
         const uint32_t a = (uint32_t)__cvta_generic_to_shared(&full_bar[tt % NSLOT]);
         const uint32_t parity = (uint32_t)((tt / NSLOT) & 1);
         uint32_t ok = 0;
-        while (!ok)
-          asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                       : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        while (!ok)                                               /* the hint lets the hardware park the warp */
+          asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                       : "=r"(ok) : "r"(a), "r"(parity), "r"(20000u) : "memory");
       }
       const bool cached = (MC != 0) && tt < mtiles;
 #pragma unroll
       for (int gg = 0; gg < GPW; ++gg) {
-        uint8_t* ff = fifo + (w * GPW + gg) * HALF_B;
+        uint16_t* ff = fifo + (w * GPW + gg) * HALF_B;
         /* survivors of the tile for this group: the cached exact-union mask, or the FP32 test against the group box */
         uint32_t bal[NR32];
         if (MC == 2 && cached) {
-          const uint32_t mw[4] = {mnext[gg].x, mnext[gg].y, mnext[gg].z, mnext[gg].w};
-#pragma unroll
-          for (int r = 0; r < NR32; ++r) bal[r] = mw[r];
-          if (tt + 1 < mtiles) mnext[gg] = __ldg(mrow + (size_t)(tt + 1) * NGRP + (w * GPW + gg));
+          const uint4 mw = mstage[(tt % NSLOT) * NGRP + (w * GPW + gg)];
+          bal[0] = mw.x;
+          if (NR32 > 1) bal[1 % NR32] = mw.y;
+          if (NR32 > 2) bal[2 % NR32] = mw.z;
+          if (NR32 > 3) bal[3 % NR32] = mw.w;
         } else {
 #pragma unroll
           for (int r = 0; r < NR32; ++r) {
@@ -687,20 +696,23 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
 #pragma unroll
         for (int r = 0; r < NR32; ++r) {
           pos[r] = tl + __popc(bal[r] & lt_mask);
-          if ((bal[r] >> lane) & 1u) ff[pos[r]] = (uint8_t)(r * 32 + lane);
+          if ((bal[r] >> lane) & 1u) ff[pos[r]] = (uint16_t)((sb + r * 32 + lane) * 16);
           tl += __popc(bal[r]);
         }
         __syncwarp();
-        /* quads; the last one may be partial (idle lanes re-read its first candidate with weight 0) */
+        /* full quads, then one partial quad (idle lanes re-read its first candidate with weight 0) */
         uint32_t nibs = 0u;                                       /* lane q: the 4 union bits of quad q */
-        const int nq = (tl + 3) >> 2;
+        const int nfull = tl >> 2;
+        const uint16_t* fq = ff + tig;
 #pragma unroll 1
-        for (int q = 0; q < nq; ++q) {
-          const int i = 4 * q + tig;
-          const bool act = i < tl;
-          const uint32_t kb = (uint32_t)sb + ff[act ? i : 4 * q];
-          const uint32_t nib = quad(gg, kb, act);
+        for (int q = 0; q < nfull; ++q) {
+          const uint32_t nib = quad(gg, fq[4 * q], true);
           if (MC == 1) nibs = (lane == q) ? nib : nibs;
+        }
+        if (tl & 3) {
+          const bool act = 4 * nfull + tig < tl;
+          const uint32_t nib = quad(gg, ff[act ? 4 * nfull + tig : 4 * nfull], act);
+          if (MC == 1) nibs = (lane == nfull) ? nib : nibs;
         }
         if (MC == 1 && cached) {
           /* exact union of the group's neighbour sets for this tile: the box mask minus the candidates that hit no home */
@@ -809,6 +821,21 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
     }
   }
 
+#ifdef CCAKE_PAIR_PROF
+  {
+    __shared__ unsigned int p_max, p_sum;
+    if (tid == 0) { p_max = 0; p_sum = 0; }
+    __syncthreads();
+    if (lane == 0) { atomicMax(&p_max, prof_quads); atomicAdd(&p_sum, prof_quads); }
+    __syncthreads();
+    if (tid == 0) {
+      const int base = (MC == 1) ? 0 : 4;
+      atomicAdd(&g_pair_prof[base + 0], (unsigned long long)p_sum);
+      atomicAdd(&g_pair_prof[base + 1], (unsigned long long)p_max * NW);
+      atomicAdd(&g_pair_prof[base + 2], 1ull);
+    }
+  }
+#endif
   /* epilogue: the sums of every home go through shared memory (the ring is no longer needed) so that one thread
      finishes one home particle and the stores are coalesced */
   __syncthreads();
