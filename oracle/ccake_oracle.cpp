@@ -26,9 +26,15 @@
  * Parity pins (tests/test_oracle_*.py): kernel normalisation and gradient (Eq. 63, 77, 79), brute-force
  * neighbour lists, partition of unity, conformal EoS identities and round trip (App. A), table exactness for
  * multilinear functions, pairwise momentum/charge conservation, dS/dx0 = dN_q/dx0 = 0 for ideal flow (Eq. 105-106),
- * ideal Gubser flow (Eq. 116-120), Bjorken ideal/shear/bulk ODEs, viscous Gubser ODE (Eq. 112), RK order.
- * PARITY UNPINNED: DNMR extra terms beyond their minimal-IS limit, the moving-frame part of
- * diffusion.
+ * ideal Gubser flow (Eq. 116-120), Bjorken ideal/shear/bulk ODEs, viscous Gubser ODE (Eq. 112), RK order;
+ * tests/test_oracle_pins_dissipative.py: every DNMR second-order term (boost-invariant DNMR ODEs in 2+1D and 3+1D,
+ * hand-evaluated tensors on a linear flow and on a rotating disc), the moving-frame part of diffusion (Lorentz
+ * covariance of a fluid with a transverse gradient, Christoffel term on the Bjorken slab, normal modes of a boosted
+ * fluid), the hyperbolic energy and work totals (energy-momentum conservation, static fluid in hyperbolic
+ * coordinates) and the (div v) accumulator (finite difference of sigma*).  A mutation run (19 single-line changes of
+ * those terms) is caught by these tests.
+ * PARITY UNPINNED: none of the terms on the path; the bulk sector has only the boost-invariant ODEs (the
+ * paper itself has no other analytic check for bulk, :1051).
  *
  * Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  OpenMP is used only as
  * "parallel for" over the particle index a of gather loops, so results do not depend on the thread count.
