@@ -47,11 +47,30 @@ def flop_grad_per_pair(D, visc, diff):
     return 34.0 + 3.0 * terms
 
 
-FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
+FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-partitions x 16 DFMA lanes x 2 flop x 1.965 GHz
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# capture of this command (profiles/r1j_README.md); only valid for the workload it was taken on
-NCU_TRAFFIC_BYTES = {("C4", "grad"): 2.068537e9 + 0.474270e9, ("C4", "smooth"): 0.538632e9 + 0.310808e9}
+
+def ncu_traffic(config, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a pair kernel, read from the committed ncu --set full
+    summary of this round (profiles/r2_traffic.json: written from the capture, with the command that made it); None
+    when the file has no entry for this workload — never a constant pasted into this script."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        with open(p) as fh:
+            return json.load(fh).get(config, {}).get(kernel)
+    except Exception:
+        return None
+
+
+_TABLES = {}
+
+
+def shared_table():
+    """C3, C4 and C4' read the same 100x32^3x11 table: build it once per process."""
+    from paper_2511_22852_b200 import workloads as W
+    if "t" not in _TABLES:
+        _TABLES["t"] = W.make_eos_table(100, 32, with_wq=True)
+    return _TABLES["t"]
 
 
 def make_workload(name, rank=0, tiles=None):
@@ -61,11 +80,13 @@ def make_workload(name, rank=0, tiles=None):
     if name == "C2":
         return W.config_c2()
     if name == "C3":
-        return W.config_c3(tile0=4 * rank)
+        return W.config_c3(tile0=4 * rank, table=shared_table())
     if name == "C4":
-        return W.config_c4(K=tiles or 10, tile0=10 * rank)
+        return W.config_c4(K=tiles or 10, tile0=10 * rank, table=shared_table())
     if name == "C5":
         return W.config_c5(tile0=13 * rank)
+    if name == "C4p":
+        return W.config_c4p(table=shared_table())
     raise SystemExit(f"unknown config {name}")
 
 
@@ -138,6 +159,8 @@ def oracle_sample(name):
         return W.config_c4(K=1), "1 of 10 event tiles (198,400 particles), 1 RK2 step"
     if name == "C5":
         return W.config_c5(K=1, n_eta=5), "1 of 13 event tiles cut to 5 rapidity slices (353,780 particles), 1 RK2 step"
+    if name == "C4p":
+        return W.config_c4p(n_side=60), "a 60^3 sub-lattice of the 126^3 probe (216,000 particles), 1 RK2 step"
     w = make_workload(name)
     return w, f"whole workload ({w.n} particles), 1 RK2 step"
 
@@ -185,6 +208,7 @@ def workload_text(name):
         "C3": "BASELINE.json configs[2]: (2+1)D viscous hyperbolic, 217,156 particles (4 event tiles), IS shear+bulk+diffusion, table 100x32^3x11, RK2",
         "C4": "BASELINE.json configs[3]: (3+1)D viscous hyperbolic, 1,984,000 particles (10 event tiles of 80x80x31), DNMR shear+bulk+BSQ diffusion, table 100x32^3x11, h=0.3, RK2",
         "C5": "BASELINE.json configs[4]: (3+1)D viscous hyperbolic, 19,316,388 particles (13 event tiles of 266x266x21), IS shear+bulk+diffusion, table 200x48^3x11, RK2",
+        "C4p": "SURVEY.md §8(d) C4' sparse probe: (3+1)D viscous hyperbolic, 2,000,376 particles on a simple cubic 126^3 lattice (spacing 0.2244, ~80 neighbours at h=0.3), C4 physics, table 100x32^3x11, RK2",
     }[name]
 
 
@@ -203,6 +227,48 @@ def algorithmic_bytes_per_particle(D, visc, bulk, diff, ncols):
     grad = 8 * (D + n_pair_in + n_grad_out)
     eom = 8 * (n_grad_out + 14 + 2 * n_state + n_state)    # sums, thermo, y_cur, y_base; write y_out
     return {"sort": sort, "smooth": smooth, "thermo": thermo + gather, "grad": grad, "eom": eom}
+
+
+def short_run(name, steps, device, hbm):
+    """A short device-timed run of another config (3 warm-up steps, `steps` timed steps from the loaded state, CUDA events
+    on the library's stream): ms per RK2 step, updates/s, neighbours, the substep's algorithmic HBM fraction."""
+    import torch
+    from paper_2511_22852_b200 import binding as B
+    w = make_workload(name)
+    p = w.params
+    stream = torch.cuda.Stream()
+    sim = B.Ccake(device=device, stream=stream.cuda_stream, **p)
+    dev = torch.device("cuda", device)
+    if w.table is not None:
+        sim.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], torch.as_tensor(w.table["data"], device=dev))
+    dfields = {k: torch.as_tensor(np.ascontiguousarray(v), device=dev) for k, v in w.fields.items()}
+    sim.load_particles(dfields)
+    npairs = float(sim.conserved_totals()[14])
+    for _ in range(3):
+        sim.step(1)
+    sim.synchronize(strict=False)
+    sim.load_particles(dfields)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record()
+        for _ in range(steps):
+            sim.step(1)
+        e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    rc = sim.synchronize(strict=False)
+    sim.close()
+    D = p["dim"]
+    on = p["eom"] != 0
+    ncols = len(w.table["col_ids"]) if w.table is not None else 0
+    bpp = algorithmic_bytes_per_particle(D, on and bool(p["flags"] & 1), on and bool(p["flags"] & 2), on and bool(p["flags"] & 4), ncols)
+    nsub = 2 if p["integrator"] == 2 else 4
+    del dfields
+    torch.cuda.empty_cache()
+    return {"particles": w.n, "steps": steps, "ms_per_step": ms, "updates_per_s": w.n / (ms * 1e-3),
+            "neighbours_per_particle": npairs / w.n, "substep_hbm_frac": sum(bpp.values()) * w.n * nsub / (ms * 1e-3) / 1e9 / hbm,
+            "rc": rc}
 
 
 def run_ours(args):
@@ -233,7 +299,8 @@ def run_ours(args):
     ids = list(w.fields.keys())
     dfields = {k: torch.as_tensor(np.ascontiguousarray(w.fields[k]), device=dev) for k in ids}
     sim.load_particles(dfields)
-    npairs = float(sim.conserved_totals()[14])          # ordered neighbour pairs, excluding self
+    npairs0 = float(sim.conserved_totals()[14])         # ordered neighbour pairs (excluding self) at the loaded state
+    fp64_peak = B.measure_fp64_peak(local) if rank == 0 else None     # DFMA chains on every SM, before the timed region
 
     def barrier():
         if world > 1:
@@ -271,6 +338,8 @@ def run_ours(args):
     n_all = float(tot_n.item())
     value = n_all * args.steps / (ms_total * 1e-3)
     totals = sim.conserved_totals()
+    npairs1 = float(totals[14])                         # ... and at the end of the timed region (the event expands)
+    npairs = 0.5 * (npairs0 + npairs1)
 
     # ---- end to end through the C ABI with HOST buffers -----------------------------------------------------
     host_in = {k: torch.empty(w.n, dtype=torch.float64).pin_memory() for k in ids}
@@ -361,12 +430,28 @@ def run_ours(args):
             if nm == "pack" or groups[nm] <= 0:
                 continue
             b = bytes_pp[nm] * w.n
+            if nm == "thermo" and w.table is not None:
+                # the 16-node stencils of neighbouring particles overlap: the gather is served by L1/L2, and what HBM has
+                # to deliver is at most the table itself, once — counted so (an upper bound of the unique bytes)
+                gather = 16 * ncols * 8 * w.n
+                table_b = float(np.prod([len(a) for a in w.table["axes"]])) * ncols * 8
+                b = b - gather + min(gather, table_b)
             kernels[nm] = {"ms": groups[nm], "alg_GB": b / 1e9, "GBps": b / (groups[nm] * 1e-3) / 1e9,
                            "hbm_frac": b / (groups[nm] * 1e-3) / 1e9 / hbm}
+            if nm == "thermo" and w.table is not None:
+                kernels[nm]["gather_GB_l2_served"] = gather / 1e9
+                kernels[nm]["note"] = "alg_GB = per-particle streams + the table once; the 1,408 B/particle stencil gather is L1/L2-served"
         kernels["smooth"]["TFLOPs"] = npairs * FLOP_SMOOTH_PER_PAIR / (groups["smooth"] * 1e-3) / 1e12
         kernels["grad"]["TFLOPs"] = npairs * fg / (groups["grad"] * 1e-3) / 1e12
         total_bytes = sum(bytes_pp.values()) * w.n
         cpu_val, cpu_ms, cores, what, _ = time_oracle(args.config, 1, 0) if not args.no_cpu else (None, None, 0, "skipped", None)
+        sim.close()
+        others = None
+        if not args.no_others and world == 1:
+            others = {}
+            for nm, st in (("C1", 20), ("C2", 20), ("C3", 10), ("C4p", 5), ("C5", 2)):
+                if nm != args.config:
+                    others[nm] = short_run(nm, st, local, hbm)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -376,11 +461,15 @@ def run_ours(args):
             "pair_interactions_per_s": npairs * 2 * nsub * args.steps * world / (ms_total * 1e-3),
             "substep_hbm_frac": total_bytes * nsub / (ms_total / args.steps * 1e-3) / 1e9 / hbm,
             "roofline": {"bound": "alu", "kernel": {"grad": "gradient pass a6", "smooth": "smoothing pass a4"}[dom],
-                         "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
-                         "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)) if args.tiles is None else None,
-                         "traffic_unit": "bytes per launch (ncu --set full, profiles/r1j_README.md)",
-                         "algorithmic_bytes": bytes_pp[dom] * w.n, "peak_source": "fp64 DFMA: 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,
+                         "peak_source": "measured in this run (ccake_measure_fp64_peak: fma.rn.f64 chains on every SM)",
+                         "peak_nominal": FP64_NOMINAL_TFLOPS,
+                         "traffic": ncu_traffic(args.config, dom) if args.tiles is None else None,
+                         "traffic_unit": "bytes per launch (ncu --set full, profiles/r2_README.md)",
+                         "algorithmic_bytes": bytes_pp[dom] * w.n,
                          "flop_per_pair": fg if dom == "grad" else FLOP_SMOOTH_PER_PAIR,
+                         "flop_convention": "algorithmic: 34 geometry + 3 per accumulated term (DESIGN.md §5); the kernel executes ~24 FP64 instructions + 6 DMMA per 32 pair evaluations",
+                         "ordered_pairs_at_load": npairs0, "ordered_pairs_after_run": npairs1,
                          "hbm_peak_GBps": hbm, "hbm_peak_source": which},
             "kernels": kernels,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
@@ -392,6 +481,7 @@ def run_ours(args):
             "freezeout_element_ms": fo_ms,
             "source_smearing": {"partons": 2000, "h_source": 1.4, "ms": src_ms,
                                 "note": "ccake_smear_sources through host buffers, incl. 63 MB device-to-host"},
+            "other_configs": others,
             "clocks": clocks,
             "status": {"rc": rc, "n_out_of_table": totals[11], "n_bad": totals[13], "x0": totals[0]},
         }
@@ -405,10 +495,11 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5", "C4p"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tiles", type=int, default=None, help="C4 only: number of event tiles (profiling runs; default 10)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs (other_configs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

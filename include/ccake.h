@@ -131,7 +131,6 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
                            const double* const axes[4], int32_t ncols, const int32_t* col_ids, double* out,
                            int32_t memspace);
 
-/* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
 /* NEXT-3 (part) of SURVEY.md §8(f): the source smearing of PAPER.md Eq. 35 (:521), the gather half of the dynamical
  * initialisation.  For every loaded particle i, at the context's current time x0 and step dx0,
  *   j^mu_i = eta_norm / (dx0 sqrt(-g)) * sum over partons k with x0 - dx0 < t[k] <= x0 of p[mu][k] W(r_i - r[.][k]; h_source),
@@ -143,6 +142,7 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
 int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
                         const double* t, double h_source, double eta_norm, double* const j[4], int32_t memspace);
 
+/* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
 int ccake_step(ccake_ctx* c, int32_t nsteps);
 
 /* Wait for the stream.  ERANGE when, since the last load, a particle left the EoS table, a per-particle solve
@@ -154,7 +154,9 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* field_ids, d
                       int64_t capacity, int32_t memspace);
 
 /* out (host) = { x0, E, P_1, P_2, P_3, S_tot, N_B, N_S, N_Q, sum m, work, n_out_of_table, max |trace pi|,
- *                n_bad, sum_a N_nb(a), 0 } at the current state (DESIGN.md §"Totals"). */
+ *                n_bad, sum_a N_nb(a), n_out_of_table_total } at the current state (DESIGN.md §"Totals").
+ * n_out_of_table counts the particles clamped to the EoS table in the evaluation at the current state;
+ * n_out_of_table_total sums that count over every substep of every step since the last load. */
 int ccake_conserved_totals(ccake_ctx* c, double out[16]);
 
 /* Test hook: neighbour sets {b != a : r_ab^2 < (2h)^2} of the current state, ORIGINAL indices, ascending per
@@ -163,7 +165,9 @@ int ccake_conserved_totals(ccake_ctx* c, double out[16]);
 int ccake_read_neighbors(ccake_ctx* c, int64_t* counts, int64_t* offsets, int32_t* list, int64_t cap);
 
 /* Test hook for sizes where lists do not fit: per particle (original order) the order-free hash
- * sum_b mix64(b) mod 2^64 over its neighbour set, mix64 = the splitmix64 finaliser of (b + 1).  Host pointer. */
+ * sum_b mix64(b) mod 2^64 over its neighbour set, mix64 = the splitmix64 finaliser of (b + 1).  Host pointer.
+ * The sets are the ones the smoothing pass itself used: the hash is accumulated by a test instantiation of the pair
+ * kernel (same candidate lists, tiles, culling and exact test), not by a separate walk. */
 int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity);
 
 /* Measurement hook: average device time in ms of each kernel group over the substeps run since the last
@@ -175,7 +179,17 @@ int ccake_enable_timing(ccake_ctx* c, int32_t on);
  * no synchronisation); the counter is then reset. */
 int ccake_launch_count(ccake_ctx* c, int64_t* out);
 
+/* Measurement hook: the FP64 rate of the device, TFLOP/s (2 flop per fused multiply-add), from chains of independent
+ * fma.rn.f64 on every SM, best of 5 launches timed with CUDA events on the default stream.  bench.py divides the
+ * pair passes' achieved flop rate by this number.  Needs no context. */
+int ccake_measure_fp64_peak(int32_t device, double* tflops);
+
 const char* ccake_last_error(const ccake_ctx* c);
+
+/* Test knobs (environment, read by ccake_load_particles): CCAKE_CAND_CAP = entries per pair block of the candidate
+ * lists (0: none — every block lists its candidates inside the pass), CCAKE_MASK_TILES = tiles per block whose hit
+ * masks the smoothing pass keeps for the gradient pass (0: none).  They force the paths a production run takes only
+ * when a block's neighbourhood outgrows its list or when device memory is short. */
 
 #ifdef __cplusplus
 }

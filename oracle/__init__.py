@@ -65,6 +65,7 @@ def lib():
         L.oracle_eos_closed_form.argtypes = [C.POINTER(Params), dbl, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_eos_forward.argtypes = [C.POINTER(Params), dbl, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_eos_table_lookup.argtypes = [vp, dbl, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32)]
+        L.oracle_set_sources.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
         L.oracle_smear_sources.argtypes = [vp, C.c_int64, C.POINTER(vp), C.POINTER(vp), vp, dbl, dbl, C.POINTER(vp)]
         _lib = L
     return _lib
@@ -170,6 +171,18 @@ class Oracle:
         self._chk(lib().oracle_smear_sources(self._h, t.size, pp, rr, t.ctypes.data, float(h_source), float(eta_norm), oo),
                   "oracle_smear_sources")
         return out
+
+    def set_sources(self, I=None, Iq=None):
+        """oracle_set_sources (Eq. 38): I [4, n] contravariant I^mu, Iq [3, n]; None clears."""
+        keep = []
+
+        def ptrs(a, k):
+            if a is None:
+                return None
+            a = np.ascontiguousarray(a, dtype=np.float64).reshape(k, self.n)
+            keep.append(a)
+            return (C.c_void_p * k)(*[a[m].ctypes.data for m in range(k)])
+        self._chk(lib().oracle_set_sources(self._h, ptrs(I, 4), ptrs(Iq, 3)), "oracle_set_sources")
 
     def eos_table_lookup(self, s, n):
         out = (C.c_double * 11)()

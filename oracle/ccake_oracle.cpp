@@ -15,6 +15,9 @@
  *   Step 7  conserved totals              §5.6.5 :1049-1063
  *   extra   applicability diagnostics     Eq. 58-61 :797-805 (Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1; pinned on Bjorken)
  *   extra   source smearing               Eq. 35 :521 (pinned: single parton, partition of unity, window, linearity)
+ *   extra   source terms I^nu, I_q        Eq. 38 :623, Eq. 42-44 :645-649, Eq. 96 :1003 (pinned: heating and push of a
+ *                                         uniform fluid, Bjorken ODE with a source, energy balance of a moving fluid,
+ *                                         exact momentum / charge balance)
  *   extra   freeze-out surface element    Eq. 145-148 :1466-1482 (d_mu eps, n_mu, |d sigma|; pinned on Bjorken, Gubser)
  *
  * There is no blocking, fusion or reordering: loops are gather form (for a { for b }), the per-particle linear
@@ -97,6 +100,7 @@ struct Derived {
   std::vector<int64_t> nb_off;
   std::vector<int32_t> nb_idx;
   int64_t n_oob = 0;
+  int64_t n_oob_steps = 0;   /* summed over the evaluations of rk_step since the last load */
 };
 
 struct Table {
@@ -118,6 +122,7 @@ struct oracle_ctx {
   State rate;
   Derived d;
   Table tab;
+  std::vector<double> src[7];   /* I^0..I^3, I_B, I_S, I_Q per particle (empty: zero), Eq. 38 */
   std::string err;
 };
 
@@ -672,7 +677,7 @@ static int state_id_of_pi(int i, int j) {
 /* Assemble and solve the linear system of one particle; write the time derivatives into k.
    Returns false on a singular system. */
 static bool eom_particle(const oracle_params& P, const Geometry& g, const State& y, const Derived& d, int64_t a,
-                         double x0, State& k, double& theta_out, double diag_out[4]) {
+                         double x0, State& k, double& theta_out, double diag_out[4], const double Isrc[7]) {
   const int D = P.dim;
   const Unknowns U = unknown_layout(D);
   const int NU = U.nu;
@@ -810,7 +815,8 @@ static bool eom_particle(const oracle_params& P, const Geometry& g, const State&
     const double pit0_lo = g.glo[i] * ds.pit[0][i];
     const Aff dpit0_lo = Aff(g.dglo[i] * ds.pit[0][i]) + g.glo[i] * dpit[0][i];
     const Aff lhs = ulo[i] * dC + Cc * dulo[i] + (1.0 / gam) * dpit0_lo - (pit0_lo / (gam * gam)) * du[0];
-    eq.push_back(lhs - Aff(g.sqrtg * (d.FP[i - 1][a] - d.FB[i - 1][a])));
+    /* source, Eq. 38 / 43: + sqrt(-g) I_i / sigma* = I_i / (gamma sigma), I_i = g_ii I^i */
+    eq.push_back(lhs - Aff(g.sqrtg * (d.FP[i - 1][a] - d.FB[i - 1][a]) + g.glo[i] * Isrc[i] / (gam * sig)));
   }
   /* entropy, Eq. 96 (:1003) with I = 0:  u^0 sigma T dS + u^0 sigma mu_q dN_q = -Pi theta + pi^mu_nu nabla_mu u^nu */
   {
@@ -822,12 +828,15 @@ static bool eom_particle(const oracle_params& P, const Geometry& g, const State&
         const double pi_m_n = sig * ds.pit[m][n] * g.glo[n];
         if (pi_m_n != 0.0) rhs = rhs + pi_m_n * CD[m][n];
       }
+    double uI = 0.0;                          /* u_mu I^mu, Eq. 96 */
+    for (int m = 0; m < 4; ++m) uI += ulo[m] * Isrc[m];
+    rhs = rhs + Aff(uI);
     eq.push_back(lhs - rhs);
   }
   /* charge:  d/dx0 [ N_q + J~^0_q / gamma ] = - sqrt(-g) FK_q */
   for (int q = 0; q < NQ; ++q) {
     const Aff lhs = dN[q] + (1.0 / gam) * dJt[q][0] - (ds.Jt[q][0] / (gam * gam)) * du[0];
-    eq.push_back(lhs + Aff(g.sqrtg * d.FK[q][a]));
+    eq.push_back(lhs + Aff(g.sqrtg * d.FK[q][a] - Isrc[4 + q] / (gam * sig)));     /* Eq. 44: + I_q */
   }
   /* bulk (Eq. 49 / Eq. 52 row 1 in terms of Pi~ = Pi/sigma, D sigma = -sigma theta):
      tau_Pi sigma gamma dPi~ = -Pi - zeta theta + (tau_Pi - delta_PiPi) Pi theta + lambda_Pipi pi^{mn} sigma_{mn} */
@@ -1031,8 +1040,10 @@ static int evaluate(oracle_ctx* c, const State& y, double x0, Derived& d, State&
   int bad = 0;
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : bad)
   for (int64_t a = 0; a < N; ++a) {
-    double th = 0.0, dg[4] = {0.0, 0.0, 0.0, 0.0};
-    if (!eom_particle(P, g, y, d, a, x0, k, th, dg)) bad++;
+    double th = 0.0, dg[4] = {0.0, 0.0, 0.0, 0.0}, Isrc[7];
+    for (int m = 0; m < 7; ++m) Isrc[m] = c->src[m].empty() ? 0.0 : c->src[m][a];
+    if (P.dim == 2) Isrc[3] = 0.0;
+    if (!eom_particle(P, g, y, d, a, x0, k, th, dg, Isrc)) bad++;
     d.theta[a] = th;
     for (int i = 0; i < 4; ++i) d.diag[i][a] = dg[i];
     for (int i = 0; i < P.dim; ++i) d.fm[i][a] = g.sqrtg * (d.FP[i][a] - d.FB[i][a]);
@@ -1064,8 +1075,10 @@ static int rk_step(oracle_ctx* c) {
     /* midpoint: k1 = f(y0, x0); y_half = y0 + dt/2 k1; k2 = f(y_half, x0 + dt/2); y1 = y0 + dt k2 */
     State k1, k2, yh;
     if ((rc = evaluate(c, c->y, x0, d, k1))) return rc;
+    d.n_oob_steps += d.n_oob;
     axpy(c->y, 0.5 * dt, k1, yh, N);
     if ((rc = evaluate(c, yh, x0 + 0.5 * dt, d, k2))) return rc;
+    d.n_oob_steps += d.n_oob;
     State y1;
     axpy(c->y, dt, k2, y1, N);
     c->y = y1;
@@ -1073,12 +1086,16 @@ static int rk_step(oracle_ctx* c) {
     /* classical RK4 */
     State k1, k2, k3, k4, t;
     if ((rc = evaluate(c, c->y, x0, d, k1))) return rc;
+    d.n_oob_steps += d.n_oob;
     axpy(c->y, 0.5 * dt, k1, t, N);
     if ((rc = evaluate(c, t, x0 + 0.5 * dt, d, k2))) return rc;
+    d.n_oob_steps += d.n_oob;
     axpy(c->y, 0.5 * dt, k2, t, N);
     if ((rc = evaluate(c, t, x0 + 0.5 * dt, d, k3))) return rc;
+    d.n_oob_steps += d.n_oob;
     axpy(c->y, dt, k3, t, N);
     if ((rc = evaluate(c, t, x0 + dt, d, k4))) return rc;
+    d.n_oob_steps += d.n_oob;
     State y1 = c->y;
     for (int f = 0; f < OF_NSTATE; ++f) {
       if (f == OF_MASS) continue;
@@ -1144,6 +1161,8 @@ int oracle_load_particles(oracle_ctx* c, int64_t n, int32_t nfields, const int32
     c->y.f[OF_JB3].assign(n, 0.0); c->y.f[OF_JS3].assign(n, 0.0); c->y.f[OF_JQ3].assign(n, 0.0);
   }
   c->N = n;
+  for (int m = 0; m < 7; ++m) c->src[m].clear();
+  c->d.n_oob_steps = 0;
   c->x0 = c->P.x0_start;
   c->loaded = true;
   c->derived_valid = false;
@@ -1291,7 +1310,7 @@ int oracle_conserved_totals(oracle_ctx* c, double out[16]) {
   }
   out[0] = c->x0; out[1] = E; out[2] = Pm[0]; out[3] = Pm[1]; out[4] = Pm[2]; out[5] = St;
   out[6] = Nq[0]; out[7] = Nq[1]; out[8] = Nq[2]; out[9] = M; out[10] = work; out[11] = (double)d.n_oob;
-  out[12] = trace; out[13] = 0.0; out[14] = npairs; out[15] = 0.0;
+  out[12] = trace; out[13] = 0.0; out[14] = npairs; out[15] = (double)d.n_oob_steps;
   return ORACLE_OK;
 }
 
@@ -1338,6 +1357,18 @@ int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double o
   const Thermo th = eos_table(c->tab, s, n);
   thermo_to_out(th, out);
   if (oob) *oob = th.oob;
+  return ORACLE_OK;
+}
+
+int oracle_set_sources(oracle_ctx* c, const double* const I[4], const double* const Iq[3]) {
+  if (!c) return ORACLE_EINVAL;
+  if (!c->loaded) return ORACLE_ESTATE;
+  for (int m = 0; m < 7; ++m) {
+    const double* col = (m < 4) ? (I ? I[m] : nullptr) : (Iq ? Iq[m - 4] : nullptr);
+    if (col) c->src[m].assign(col, col + c->N);
+    else c->src[m].clear();
+  }
+  c->derived_valid = false;
   return ORACLE_OK;
 }
 

@@ -94,6 +94,15 @@ int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double o
 int oracle_smear_sources(oracle_ctx* c, int64_t np, const double* const p[4], const double* const r[3], const double* t,
                          double h_source, double eta_norm, double* const j[4]);
 
+/* Source terms of the conservation equations, Eq. 38 (:623), Eq. 42-44 (:645-649), Eq. 96 (:1003):
+ * nabla_mu T^{mu nu} = I^nu, nabla_mu N^mu_q = I_q.  I: 4 columns (contravariant I^mu per particle, e.g. the j^mu of
+ * oracle_smear_sources), Iq: 3 columns; n doubles each; a NULL array or NULL column means zero.  They stay in force for
+ * every evaluation until set again.  In the conservative per-particle form of Step 5:
+ *   d/dx0 [ C u_i + pi~^0_i / gamma ] = sqrt(-g) (FP_i - FB_i) + I_i / (gamma sigma),       I_i = g_ii I^i
+ *   d/dx0 [ N_q + J~^0_q / gamma ]     = -sqrt(-g) FK_q + I_q / (gamma sigma)
+ *   gamma sigma (T dS + mu_q dN_q)     = u_mu I^mu - Pi theta + pi^mu_nu nabla_mu u^nu                          */
+int oracle_set_sources(oracle_ctx* c, const double* const I[4], const double* const Iq[3]);
+
 #ifdef __cplusplus
 }
 #endif

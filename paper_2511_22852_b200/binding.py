@@ -34,7 +34,7 @@ EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
-           "ccake_last_error"]
+           "ccake_measure_fp64_peak", "ccake_last_error"]
 
 
 class Params(C.Structure):
@@ -84,10 +84,20 @@ def lib():
         L.ccake_kernel_times.argtypes = [vp, C.POINTER(C.c_double)]
         L.ccake_enable_timing.argtypes = [vp, i32]
         L.ccake_launch_count.argtypes = [vp, C.POINTER(i64)]
+        L.ccake_measure_fp64_peak.argtypes = [i32, C.POINTER(C.c_double)]
         L.ccake_last_error.argtypes = [vp]
         L.ccake_last_error.restype = C.c_char_p
         _lib = L
     return _lib
+
+
+def measure_fp64_peak(device=0) -> float:
+    """ccake_measure_fp64_peak: TFLOP/s of the device's FP64 pipe (DFMA chains on every SM)."""
+    out = C.c_double(0.0)
+    rc = lib().ccake_measure_fp64_peak(int(device), C.byref(out))
+    if rc != 0:
+        raise CcakeError("ccake_measure_fp64_peak", rc, "")
+    return float(out.value)
 
 
 def make_params(**kw) -> Params:

@@ -229,7 +229,7 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   if ((rc = mark(c))) return rc;
   /* a5 */
   cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
-  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, c->tb, Ycur, np, c->so, c->status);
+  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, c->tb, Ycur, np, c->so, c->status, rk_in.update);
   if ((rc = mark(c))) return rc;
   /* a6 */
   launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
@@ -462,10 +462,6 @@ __global__ void scatter_diff_kernel(const double* __restrict__ x, const double* 
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) dst[orig[perm[i]]] = scale * (x[i] - (y ? y[i] : 0.0));
 }
-__global__ void gather_load_kernel(const double* __restrict__ src, int64_t n, double* __restrict__ dst) {
-  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (i < n) dst[i] = src[i];
-}
 __global__ void fill_kernel(double* __restrict__ dst, int64_t n, double v) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) dst[i] = v;
@@ -516,6 +512,31 @@ __global__ void neighbour_walk_kernel(int64_t n, KParams kp, const Grid* __restr
     }
   }
   if (mode == 0) hash_out[ao] = hsum;
+}
+
+
+/* ------------------------------------------------------------------------ measurement hook: FP64 peak ---- */
+/* 8 independent fma.rn.f64 chains per thread (inline PTX, so nothing is folded or reordered), every SM loaded with
+   8 blocks of 256 threads: the rate at which the SM's FP64 pipe retires DFMAs, the roofline the pair passes are
+   measured against.  The same pipe executes the FP64 tensor-core MMAs at the same flop rate. */
+__global__ void __launch_bounds__(256) fp64_peak_kernel(int iters, double* out) {
+  double a0 = threadIdx.x * 1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 1.0000001, c = 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a0) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a1) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a2) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a3) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a4) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a5) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a6) : "d"(m), "d"(c));
+      asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a7) : "d"(m), "d"(c));
+    }
+  }
+  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == 123.456) out[0] = s;
 }
 
 }  // namespace
@@ -898,7 +919,7 @@ int ccake_synchronize(ccake_ctx* c) {
   Status s;
   CK(cudaMemcpy(&s, c->status, sizeof(Status), cudaMemcpyDeviceToHost));
   if (s.n_bad) { c->err = "singular per-particle system or NaN"; return CCAKE_ERANGE; }
-  if (s.n_oob) { c->err = "particles outside the EoS table (clamped)"; return CCAKE_ERANGE; }
+  if (s.n_oob || s.n_oob_total) { c->err = "particles outside the EoS table (clamped)"; return CCAKE_ERANGE; }
   return CCAKE_OK;
 }
 
@@ -1016,7 +1037,7 @@ int ccake_conserved_totals(ccake_ctx* c, double out[16]) {
   for (int k = 0; k < 16; ++k) out[k] = 0.0;
   out[0] = c->x0; out[1] = t[0]; out[2] = t[1]; out[3] = t[2]; out[4] = t[3]; out[5] = t[4];
   out[6] = t[5]; out[7] = t[6]; out[8] = t[7]; out[9] = t[8]; out[10] = t[9]; out[11] = (double)s.n_oob;
-  out[12] = t[13]; out[13] = (double)s.n_bad; out[14] = t[10]; out[15] = 0.0;
+  out[12] = t[13]; out[13] = (double)s.n_bad; out[14] = t[10]; out[15] = (double)s.n_oob_total;
   return CCAKE_OK;
 }
 
@@ -1075,6 +1096,38 @@ int ccake_neighbor_hash(ccake_ctx* c, uint64_t* out, int64_t capacity) {
   cudaFree(d);
   if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return CCAKE_ECUDA; }
   return CCAKE_OK;
+}
+
+int ccake_measure_fp64_peak(int32_t device, double* tflops) {
+  if (!tflops) return CCAKE_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return CCAKE_ECUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return CCAKE_ECUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return CCAKE_ECUDA;
+  double* out = nullptr;
+  if (cudaMalloc(&out, sizeof(double)) != cudaSuccess) return CCAKE_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
+  fp64_peak_kernel<<<blocks, threads>>>(64, out);                 /* warm-up */
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0);
+    fp64_peak_kernel<<<blocks, threads>>>(iters, out);
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+    if (ms > 0.f) best = std::max(best, flop / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  *tflops = best;
+  return (best > 0.0 && cudaGetLastError() == cudaSuccess) ? CCAKE_OK : CCAKE_ECUDA;
 }
 
 int ccake_launch_count(ccake_ctx* c, int64_t* out) {

@@ -135,7 +135,7 @@ struct Sorted {
 struct Status {
   unsigned long long n_oob;      /* particles outside the EoS table in the latest thermo pass */
   unsigned long long n_bad;      /* singular solves / NaN since the last load                 */
-  unsigned long long n_oob_total;
+  unsigned long long n_oob_total;   /* ... summed over every substep of every step since the last load    */
 };
 
 }  // namespace ccake

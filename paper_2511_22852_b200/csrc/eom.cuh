@@ -267,7 +267,7 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int64_t a = so.perm[i];
-  const double* __restrict__ Y = rk.Ycur;
+  const double* Y = rk.Ycur;          /* may alias rk.Yout (RK4 stages 2, 3: own slot read, then written): no __restrict__ */
   EomIn in;
   load_u(kp, gm, Y, npad, a, in.u);
   in.gam = in.u[0];
@@ -280,7 +280,7 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   in.sig = so.sigma[i]; in.sst = so.sigma_star[i]; in.s = so.s[i];
   in.T = so.T[i]; in.p = so.p[i]; in.e = so.e[i]; in.cs2 = so.cs2[i]; in.ws = so.ws[i];
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) { in.mu[q] = so.mu[q][i]; in.wq[q] = kp.diff || kp.eos_kind == 0 ? so.wq[q][i] : so.wq[q][i]; }
+  for (int q = 0; q < NQ; ++q) { in.mu[q] = so.mu[q][i]; in.wq[q] = so.wq[q][i]; }
   /* transport coefficients, §5.3 (:732-769), DESIGN reading 11 */
   {
     const double w = in.e + in.p;

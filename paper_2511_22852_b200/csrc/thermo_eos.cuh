@@ -177,7 +177,7 @@ eos_invert_kernel(KParams kp, InvertArgs a, int64_t nodes, double* __restrict__ 
 struct Dissip { double pit[4][4], Jt[NQ][4], bulkt; };
 
 template <int D>
-__device__ __forceinline__ void load_dissip(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad,
+__device__ __forceinline__ void load_dissip(const KParams& kp, const Geom& gm, const double* Y, int64_t npad,
                                             int64_t a, const double u[4], Dissip& ds) {
   const double gam = u[0];
   const double G[4] = {0.0, 1.0, 1.0, gm.G3};
@@ -220,7 +220,7 @@ __device__ __forceinline__ void load_dissip(const KParams& kp, const Geom& gm, c
   }
 }
 
-__device__ inline void load_u(const KParams& kp, const Geom& gm, const double* __restrict__ Y, int64_t npad, int64_t a,
+__device__ inline void load_u(const KParams& kp, const Geom& gm, const double* Y, int64_t npad, int64_t a,
                               double u[4]) {
   u[1] = Y[CCAKE_U1 * npad + a];
   u[2] = Y[CCAKE_U2 * npad + a];
@@ -230,7 +230,7 @@ __device__ inline void load_u(const KParams& kp, const Geom& gm, const double* _
 
 __global__ void __launch_bounds__(128)
 thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restrict__ Y, int64_t npad, Sorted so,
-              Status* __restrict__ status) {
+              Status* __restrict__ status, int on_step) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int D = kp.D;
@@ -244,7 +244,10 @@ thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restr
   double nq[NQ];
   for (int q = 0; q < NQ; ++q) nq[q] = so.rho_star[q][i] / lab;
   const ThermoOut th = (kp.eos_kind == 0) ? eos_closed_form(kp, s, nq) : eos_table_lookup(tb, s, nq);
-  if (th.oob) atomicAdd(&status->n_oob, 1ULL);
+  if (th.oob) {                       /* clamped to the table: latest pass, and all substeps of steps since the load */
+    atomicAdd(&status->n_oob, 1ULL);
+    if (on_step) atomicAdd(&status->n_oob_total, 1ULL);
+  }
   so.gamma[i] = gam; so.sigma[i] = sig; so.s[i] = s;
   so.T[i] = th.T; so.p[i] = th.p; so.e[i] = th.e; so.cs2[i] = th.cs2; so.ws[i] = th.ws;
   for (int q = 0; q < NQ; ++q) {

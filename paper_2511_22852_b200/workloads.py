@@ -301,7 +301,8 @@ def _tiled_event(name, cfg_index, K, n_side, dx, n_hot, width, R, a, params, nst
         for q, fid in enumerate((NB, NS, NQ)):
             cols[fid].append(rho[q] * vol)
     fields = {k: np.concatenate(v) for k, v in cols.items() if v}
-    return Workload(name, params, fields, table, nsteps, dict(tiles=K, n_side=n_side, dx=dx, gap=gap))
+    deta = float(eta_nodes[1] - eta_nodes[0]) if eta_nodes is not None else 1.0
+    return Workload(name, params, fields, table, nsteps, dict(tiles=K, n_side=n_side, dx=dx, gap=gap, deta=deta))
 
 
 def viscous_params(dim, eom, dx0, x0=0.6):
@@ -329,6 +330,29 @@ def config_c4(K=10, n_side=80, n_eta=31, nsteps=50, n_hot=40, table=None, tile0=
                         tile0=tile0)
 
 
+def config_c4p(n_side=126, spacing=0.2244, nsteps=10, n_hot=40, table=None):
+    """C4': the sparse throughput probe — C4's physics and generator stretched to a simple cubic
+    lattice of n_side^3 sites with spacing 0.2244 in x, y and eta_s (2,000,376 particles, ~80 neighbours at h = 0.3 fm):
+    the regime BASELINE.json's config 4 states ("~80 neighbours"), where the substep sits near the HBM / FP64 ridge."""
+    params = viscous_params(3, 2, 0.05)
+    stretch = n_side * spacing / 8.0
+    eta = (np.arange(n_side) - 0.5 * (n_side - 1)) * spacing
+    if table is None:
+        table = make_eos_table(100, 32, with_wq=True)
+    w = _tiled_event("C4p", 6, 1, n_side, spacing, n_hot, 0.4 * stretch, 2.6 * stretch, 0.513 * stretch, params, nsteps,
+                     eta_nodes=eta / stretch * 1.0, table=table)
+    # the rapidity profile of C4 (plateau half-width 2, Gaussian tails) is evaluated on eta / stretch; the lattice itself
+    # has the cubic spacing
+    f = dict(w.fields)
+    f[R3] = np.tile(np.repeat(eta, n_side * n_side), 1)
+    vol_fix = spacing / ((eta[1] - eta[0]) / stretch)
+    for k in (S, NB, NS, NQ):
+        f[k] = f[k] * vol_fix
+    meta = dict(w.meta)
+    meta["deta"] = spacing
+    return Workload("C4p", params, f, table, nsteps, meta)
+
+
 def config_c5(K=13, n_side=266, n_eta=21, nsteps=20, n_hot=400, table=None, ns=200, nq=48, tile0=0):
     """C5: (3+1)D high-resolution Au+Au-like event tiles with baryon stopping, minimal IS, 200x48^3 table."""
     params = viscous_params(3, 1, 0.025)
@@ -337,6 +361,36 @@ def config_c5(K=13, n_side=266, n_eta=21, nsteps=20, n_hot=400, table=None, ns=2
         table = make_eos_table(ns, nq, with_wq=True)
     return _tiled_event("C5", 5, K, n_side, 0.06, n_hot, 0.5, 6.4, 0.54, params, nsteps, eta_nodes=eta,
                         stopping=True, table=table, tile0=tile0)
+
+
+def with_dissipative_state(w: Workload, seed: int, amp: float = 0.03, u_amp: float = 0.05) -> Workload:
+    """The same workload with a seeded non-equilibrium start: velocities u^i ~ N(0, u_amp) and Pi/sigma, pi^{ij}/sigma,
+    J^i_q/sigma drawn per particle as N(0, 1) times amp times the particle's equilibrium scale (energy per particle
+    for Pi and pi, charge per particle for J; eta components carry 1/tau per index).  The event tiles of C3-C5 start
+    at rest with Pi = pi = J = 0 (reading 17), where every second-order coupling multiplies numbers near zero; this
+    variant exercises them in the same launch configuration.  Draw order: u (per component), Pi, pi (11, 12, 22, 33,
+    13, 23), J (q-major)."""
+    p = w.params
+    D, tau0 = p["dim"], (p["x0_start"] if p["coords"] == 1 else 1.0)
+    rng = np.random.Generator(np.random.PCG64(SEED0 + 7919 * seed))
+    f = dict(w.fields)
+    n = w.n
+    dxyz = w.meta.get("dx", 0.1)
+    vol = tau0 * dxyz ** 2 * (w.meta.get("deta", 0.1) if D == 3 else 1.0)
+    s = f[S] / vol
+    T = np.cbrt(s / (4.0 * EOS_C0))
+    escale = 3.0 * EOS_C0 * T ** 4 * vol
+    gfac = [1.0, 1.0, 1.0 / tau0 if p["coords"] == 1 else 1.0]
+    for k in range(D):
+        f[U1 + k] = u_amp * rng.standard_normal(n) * gfac[k]
+    f[BULK] = amp * escale * rng.standard_normal(n)
+    comps = [(PI11, 0, 0), (PI12, 0, 1), (PI22, 1, 1), (PI33, 2, 2)] + ([(PI13, 0, 2), (PI23, 1, 2)] if D == 3 else [])
+    for fid, i, j in comps:
+        f[fid] = amp * escale * rng.standard_normal(n) * gfac[i] * gfac[j]
+    for q in range(3):
+        for k in range(D):
+            f[JB1 + 3 * q + k] = amp * np.abs(f[NB + q]) * rng.standard_normal(n) * gfac[k]
+    return Workload(w.name + "_neq", p, f, w.table, w.nsteps, dict(w.meta))
 
 
 def count_pairs_estimate(w: Workload) -> float:

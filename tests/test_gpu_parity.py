@@ -109,7 +109,8 @@ def test_fields_after_run(name):
     assert_fields(g, o, [B.SIGMA_STAR, B.S_DENS, B.T, B.P], TOL_RUN, name + " derived after run", elementwise=POSITIVE)
     t1g, t1o = g.conserved_totals(), o.conserved_totals()
     assert t1g[0] == pytest.approx(t1o[0], abs=1e-12)
-    assert (rc == B.ERANGE) == (t1o[11] > 0 or t0o[11] > 0) or rc == 0
+    assert (rc == B.ERANGE) == (t1o[15] > 0 or t1o[11] > 0), (rc, t1o[11], t1o[15])
+    assert t1g[15] == t1o[15] and t1g[11] == t1o[11]
     dg, do = drift(t0g, t1g), drift(t0o, t1o)
     scale = np.abs(t0o[1:10]).max()
     for k in dg:
@@ -182,73 +183,6 @@ def test_runs_are_reproducible():
     for k in res[0][0]:
         assert np.array_equal(res[0][0][k], res[1][0][k])
     assert np.array_equal(res[0][1], res[1][1])
-
-
-def _sampled_tile_parity(w, tb, t, nsteps):
-    """GPU on the whole tiled workload, oracle on event tile t alone (the very same coordinates and fields, sliced
-    out of the full input; tiles are independent: gaps > 2h + twice the run's reach).  Neighbour counts bit-exact,
-    smoothed densities 1e-11 element by element, thermodynamics 1e-11, gradient sums 1e-10, and every evolved
-    field 1e-8 after nsteps RK steps (nsteps = 0: one evaluation only)."""
-    K = w.meta["tiles"]
-    nt = w.n // K
-    sl = slice(t * nt, (t + 1) * nt)
-    g = B.from_workload(w)
-    o = O.Oracle(**w.params)
-    o.load_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"], tb["data"])
-    o.load_particles({k: np.ascontiguousarray(v[sl]) for k, v in w.fields.items()})
-
-    def compare(ids, tol, what, elementwise=()):
-        fg, fo = g.read_fields(ids), o.read_fields(ids)
-        bad = {}
-        for k in ids:
-            a, b = fg[k][sl], fo[k]
-            assert np.all(np.isfinite(a)), (what, k)
-            if k in elementwise:
-                with np.errstate(divide="ignore", invalid="ignore"):
-                    r = np.abs(a - b) / np.abs(b)
-                r[a == b] = 0.0
-                e = float(r.max())
-            else:
-                e = norm_rel(a, b)
-            if not e <= tol:
-                bad[k] = e
-        assert not bad, f"{what}: beyond {tol:g}: {bad}"
-
-    ng = g.read_fields([B.NNB])[B.NNB][sl]
-    no = o.read_fields([O.NNB])[O.NNB]
-    assert np.array_equal(ng, no), "neighbour counts differ on the sampled tile"
-    sums = [B.SIGMA_STAR, B.S_STAR, B.RHOSTAR_B, B.RHOSTAR_S, B.RHOSTAR_Q]
-    compare(sums, TOL_SUM, "smoothing sums", elementwise=sums)
-    compare([B.T, B.P, B.E, B.MU_B, B.MU_S, B.MU_Q], TOL_SUM, "thermodynamics")
-    compare(gradient_ids(w.params), TOL_GRAD, "gradient sums")
-    if nsteps:
-        g.step(nsteps)
-        g.synchronize()
-        o.step(nsteps)
-        compare(state_ids(w.params) + [B.SIGMA_STAR, B.T, B.P], TOL_RUN, f"fields after {nsteps} RK2 steps",
-                elementwise=(B.SIGMA_STAR, B.T, B.P))
-    g.close()
-
-
-def test_full_size_c4_sampled_event_tile():
-    """BASELINE.json configs[3] at full size (1,984,000 particles, the launch configuration bench.py times), checked
-    on a sample the oracle can afford: one of its 10 event tiles, one RK2 step."""
-    tb = W.make_eos_table(100, 32, with_wq=True)
-    _sampled_tile_parity(W.config_c4(table=tb), tb, 7, 1)
-
-
-def test_full_size_c3_sampled_event_tile():
-    """BASELINE.json configs[2] at full size (217,156 particles in 4 event tiles): one tile, 3 RK2 steps."""
-    tb = W.make_eos_table(100, 32, with_wq=True)
-    _sampled_tile_parity(W.config_c3(table=tb), tb, 2, 3)
-
-
-def test_full_size_c5_sampled_event_tile():
-    """BASELINE.json configs[4] at full size (19,316,388 particles, 200x48^3 table): one evaluation (all of a1-a7
-    at the loaded state) on one of its 13 event tiles — 1.49 M particles with ~1,700 neighbours each is what the
-    oracle can do in about a minute."""
-    tb = W.make_eos_table(200, 48, with_wq=True)
-    _sampled_tile_parity(W.config_c5(table=tb), tb, 5, 0)
 
 
 def test_full_size_c2():

@@ -22,7 +22,7 @@ def _header_text():
 def test_library_builds_and_exports_every_declared_symbol():
     cuda_build.build()
     L = B.lib()
-    declared = set(re.findall(r"\b(ccake_[a-z_]+)\s*\(", re.sub(r"/\*.*?\*/", "", _header_text(), flags=re.S)))
+    declared = set(re.findall(r"\b(ccake_[a-z0-9_]+)\s*\(", re.sub(r"/\*.*?\*/", "", _header_text(), flags=re.S)))
     assert declared, "no declarations found in include/ccake.h"
     for name in declared:
         assert hasattr(L, name), f"libccake.so does not export {name}"
