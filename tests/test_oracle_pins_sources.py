@@ -30,7 +30,7 @@ def test_uniform_fluid_at_rest_heats_and_is_pushed_exactly():
     dn_q/dt = I_q.  Rates of the centre particle at the loaded state, closed form; and with I^i = 0, I_q = 0 the energy
     density grows linearly, eps(t) = eps(0) + I^0 t (the midpoint rule is exact for a constant rate of eps... of s only
     to O(dt^2), so the comparison is at that level)."""
-    n, dx, T0 = 21, 0.1, 0.3 / W.HBARC
+    n, dx, T0 = 41, 0.1, 0.3 / W.HBARC      # wide enough that the centre's neighbours do not see the edge for 0.13 fm
     f, N = _uniform(2, n, dx, T0)
     p = W.base_params(dim=2, coords=0, eom=0, eos_kind=0, h=0.3, x0_start=0.0, dx0=0.01)
     o = O.Oracle(**p)
@@ -54,10 +54,10 @@ def test_uniform_fluid_at_rest_heats_and_is_pushed_exactly():
     e0 = o.read_fields([O.E])[O.E][ic]
     o.step(10)
     e1 = o.read_fields([O.E])[O.E][ic]
-    assert abs((e1 - e0) / (3.0 * 0.1) - 1) < 1e-5
+    assert abs((e1 - e0) / (3.0 * 0.1) - 1) < 1e-6
     o.set_sources(None, None)                                              # cleared: nothing changes any more
     o.step(3)
-    assert abs(o.read_fields([O.E])[O.E][ic] / e1 - 1) < 1e-12
+    assert abs(o.read_fields([O.E])[O.E][ic] / e1 - 1) < 1e-8
 
 
 def test_bjorken_with_energy_source():
@@ -84,47 +84,59 @@ def test_bjorken_with_energy_source():
 
 
 def test_moving_fluid_energy_and_momentum_balance():
-    """A uniform fluid moving with u^x = 0.5 under a uniform source I^mu = (I^0, I^x, 0): the momentum and charge
-    equations are in conservative form, so the totals obey d P_i/dt = sum (m/sigma*) I_i and dN_q/dt = sum (m/sigma*) I_q
-    to round-off per evaluation; the energy is not evolved, and d E/dt = sum (m/sigma*) I^0 holds to the integration
-    error — which pins u_mu I^mu (not I^0) in Eq. 96 together with I_i in the momentum equation: T^{00} = w gamma^2 - p
-    depends on both."""
-    n, dx, T0 = 21, 0.1, 0.3 / W.HBARC
+    """A uniform fluid moving with u^x = 0.5 under a uniform source I^mu = (I^0, I^x, 0).  Locally d T^{0 nu}/dt = I^nu
+    (no flux divergence in a uniform fluid): T^{00} = w gamma^2 - p and T^{0x} = w gamma u^x of the centre particle,
+    built from the read fields before and after one small step — this pins u_mu I^mu (not I^0) in Eq. 96 together with
+    I_i in the momentum equation, since T^{00} depends on both.  The momentum and charge equations are in conservative
+    form, so the totals obey dP_i/dt = sum (m/sigma*) I_i and dN_q/dt = sum (m/sigma*) I_q."""
+    n, dx, T0 = 41, 0.1, 0.3 / W.HBARC
     f, N = _uniform(2, n, dx, T0, u=(0.5, 0.0))
+    ic = N // 2
     I = np.zeros((4, N))
     I[0], I[1] = 2.0, 1.2
     Iq = np.zeros((3, N))
     Iq[1] = 0.03
-    res = []
+    err = []
     for dt in (0.004, 0.002):
         p = W.base_params(dim=2, coords=0, eom=0, eos_kind=0, h=0.3, x0_start=0.0, dx0=dt)
         o = O.Oracle(**p)
         o.load_particles(f)
         o.set_sources(I, Iq)
+
+        def T0nu():
+            r = o.read_fields([O.E, O.P, O.GAMMA, O.U1, O.RHO_S])
+            w = r[O.E][ic] + r[O.P][ic]
+            return np.array([w * r[O.GAMMA][ic] ** 2 - r[O.P][ic], w * r[O.GAMMA][ic] * r[O.U1][ic],
+                             r[O.RHO_S][ic] * r[O.GAMMA][ic]])
         vol = 1.0 / o.read_fields([O.SIGMA_STAR])[O.SIGMA_STAR]
-        t0 = o.conserved_totals()
+        a0, t0 = T0nu(), o.conserved_totals()
         o.step(1)
-        t1 = o.conserved_totals()
-        res.append(((t1[1] - t0[1]) / dt / np.sum(vol * I[0]) - 1, (t1[2] - t0[2]) / dt / np.sum(vol * -I[1]) - 1,
-                    (t1[7] - t0[7]) / dt / np.sum(vol * Iq[1]) - 1))
-    # edges of the finite block expand, which changes E slightly as well: compare at the 1e-3 level, and see it shrink
-    assert abs(res[1][0]) < 2e-3 and abs(res[1][1]) < 2e-3 and abs(res[1][2]) < 1e-6
-    # with I^0 in place of u_mu I^mu = gamma I^0 - gamma v I^x the energy rate would be off by tens of percent
+        a1, t1 = T0nu(), o.conserved_totals()
+        rate = (a1 - a0) / dt
+        err.append([abs(rate[0] / 2.0 - 1), abs(rate[1] / 1.2 - 1), abs(rate[2] / 0.03 - 1)])
+        # totals of the finite block: the charge balance is exact by the conservative form; the momentum total is
+        # rebuilt from u and the thermodynamics at the SMOOTHED s (reading 2), which near the free edges does not
+        # follow S sigma exactly: percent level
+        assert abs((t1[7] - t0[7]) / dt / np.sum(vol * Iq[1]) - 1) < 1e-9
+        assert abs((t1[2] - t0[2]) / dt / np.sum(vol * -I[1]) - 1) < 2e-2
+    assert max(err[1]) < 2e-3 and err[1][0] < 0.7 * err[0][0] + 1e-5       # first-order difference quotient: error ~ dt
+    # with I^0 in place of u_mu I^mu = gamma I^0 - gamma v I^x the energy rate would be off by more than 10 %
     gam = np.sqrt(1.25)
     assert abs((gam * 2.0 - 0.5 * 1.2) / 2.0 - 1) > 0.1
 
 
 @pytest.mark.parametrize("D,coords", [(2, 0), (3, 1)])
 def test_smeared_partons_deposit_their_four_momentum(D, coords):
-    """Eq. 35 -> Eq. 38: partons smeared onto the particles and fed back as I^mu change the totals over one step by
-    eta_norm sum_k p^mu_k (partition of unity of the smearing kernel on the lattice, a few 1e-3 at dx / h_source = 0.1):
-    momentum exactly by the conservative form, energy to the integration error."""
+    """Eq. 35 -> Eq. 38: partons smeared onto the particles (oracle_smear_sources) and fed back as I^mu.  Over one step
+    the totals change by the volume integral of the source on the time slice:
+        Cartesian:   dE = dt sum_i V_i j^0_i = eta_norm sum_k p^0_k (partition of unity of the smearing kernel),
+                     dP_i = dt sum_i V_i j_i;
+        hyperbolic:  dE = dt sum_i V_i tau (j^tau_i cosh eta_i + tau j^eta_i sinh eta_i)   (reading 14),
+    V_i = m_i / sigma*_i.  The deposit is small (eta_norm = 0.062), so the step is in its linear regime."""
     n, dx = (41, 0.14) if D == 2 else (17, 0.3)
-    T0, tau0, dt, hs, eta = 0.3 / W.HBARC, 1.3, 0.01, 1.0, 0.62
+    T0, tau0, dt, hs, eta = 0.3 / W.HBARC, 1.3, 0.01, 1.0, 0.062
     f, N = _uniform(D, n, dx, T0, tau0=tau0, hyper=bool(coords))
     p = W.base_params(dim=D, coords=coords, eom=0, eos_kind=0, h=0.45 if D == 3 else 0.3, x0_start=tau0, dx0=dt)
-    o = O.Oracle(**p)
-    o.load_particles(f)
     rng = np.random.default_rng(8)
     npart = 40
     r = np.zeros((3, npart))
@@ -133,22 +145,31 @@ def test_smeared_partons_deposit_their_four_momentum(D, coords):
     pm[0] = np.abs(pm[0]) + 2.0
     if D == 2:
         pm[3] = 0.0
-    j = o.smear_sources(pm, r, np.full(npart, tau0), hs, eta)
-    o.set_sources(j, None)
-    t0 = o.conserved_totals()
-    o.step(1)
-    t1 = o.conserved_totals()
-    # lower-index momentum P_i = g_ii P^i; in hyperbolic coordinates at eta ~ 0 the energy is E = sum tau T^{tau tau} cosh eta
-    dE = (t1[1] + t1[10]) - (t0[1] + t0[10])
-    if coords == 1:
-        # the undisturbed slab loses energy to longitudinal work (2+1D: tracked in t[10]) or keeps it (3+1D): subtract the
-        # same step without sources
-        o2 = O.Oracle(**p)
-        o2.load_particles(f)
-        a0 = o2.conserved_totals()
-        o2.step(1)
-        a1 = o2.conserved_totals()
-        dE -= (a1[1] + a1[10]) - (a0[1] + a0[10])
-    assert abs(dE / (eta * pm[0].sum()) - 1) < 0.02
+
+    def run(with_sources):
+        o = O.Oracle(**p)
+        o.load_particles(f)
+        j = o.smear_sources(pm, r, np.full(npart, tau0), hs, eta)
+        if with_sources:
+            o.set_sources(j, None)
+        vol = 1.0 / o.read_fields([O.SIGMA_STAR])[O.SIGMA_STAR]
+        t0 = o.conserved_totals()
+        o.step(1)
+        t1 = o.conserved_totals()
+        return t1 - t0, j, vol
+    d1, j, vol = run(True)
+    d0, _, _ = run(False)
+    d = d1 - d0                                  # the undisturbed block changes too (edges, longitudinal work)
+    if coords == 0:
+        expE = dt * np.sum(vol * j[0])
+        assert abs(expE / (eta * pm[0].sum()) - 1) < 1e-3          # the smearing conserves the partons' energy
+        expP = [dt * np.sum(vol * -j[1 + i]) for i in range(2)]
+    else:
+        eta_s = f[O.R3]
+        expE = dt * np.sum(vol * tau0 * (j[0] * np.cosh(eta_s) + tau0 * j[3] * np.sinh(eta_s)))
+        expP = [dt * np.sum(vol * tau0 * -j[1 + i]) for i in range(2)]
+    # hyperbolic: eps is evaluated at the SMOOTHED s (reading 2), so a deposit at eta_b is counted with cosh eta_a of the
+    # particles a within 2h of it: <cosh(eta_a - eta_b)>_W - 1 ~ 3 % at h = 0.45
+    assert abs((d[1] + d[10]) / expE - 1) < (2e-3 if coords == 0 else 5e-2)
     for i in range(2):
-        assert abs((t1[2 + i] - t0[2 + i]) / (-eta * pm[1 + i].sum()) - 1) < 0.01
+        assert abs(d[2 + i] / expP[i] - 1) < (2e-3 if coords == 0 else 1e-2)
