@@ -137,10 +137,22 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
  * W the cubic spline of Eq. 77 in the context's dimension (2 h_source cut-off), sqrt(-g) = tau (hyperbolic) or 1.
  * p: 4 columns, r: 3 columns (the first `dim` are used), t: formation times — npartons doubles each; j: 4 columns of
  * n doubles in the caller's particle order; all in `memspace`.  Every parton is tested against every particle (no
- * spatial index: parton counts per step are thousands).  The state is not modified: feeding j^mu into the equations
- * of motion (I^nu, I_q) is not built. */
+ * spatial index: parton counts per step are thousands).  The state is not modified; ccake_set_sources feeds j^mu into
+ * the equations of motion. */
 int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
                         const double* t, double h_source, double eta_norm, double* const j[4], int32_t memspace);
+
+/* Rest of NEXT-3: source terms of the conservation equations, Eq. 38 (:623) nabla_mu T^{mu nu} = I^nu,
+ * nabla_mu N^mu_q = I_q, as they enter Eq. 42-44 (:645-649) and the entropy equation Eq. 96 (:1003).  I: 4 columns, the
+ * contravariant I^mu per particle (for instance the j^mu of ccake_smear_sources; I[3] is ignored when dim == 2); Iq: 3
+ * columns I_B, I_S, I_Q; n doubles each in the caller's particle order, in `memspace`.  A NULL array or column is zero;
+ * both NULL switches the sources off.  The values are copied and stay in force for every substep of every following
+ * step until set again; ccake_load_particles clears them.  In the per-particle form the kernels solve (DESIGN reading 4):
+ *   d/dx0 [C u_i + pi~^0_i / gamma] = sqrt(-g) (FP_i - FB_i) + I_i / (gamma sigma),   I_i = g_ii I^i,
+ *   d/dx0 [N_q + J~^0_q / gamma]     = -sqrt(-g) FK_q + I_q / (gamma sigma),
+ *   gamma sigma (T dS + mu_q dN_q)   = u_mu I^mu - Pi theta + pi^mu_nu nabla_mu u^nu.
+ * ESTATE before a load. */
+int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* const Iq[3], int32_t memspace);
 
 /* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
 int ccake_step(ccake_ctx* c, int32_t nsteps);

@@ -31,6 +31,7 @@ HOST, DEVICE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_smear_sources",
+           "ccake_set_sources",
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
@@ -75,6 +76,7 @@ def lib():
         L.ccake_load_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
         L.ccake_invert_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
         L.ccake_smear_sources.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp), i32]
+        L.ccake_set_sources.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), i32]
         L.ccake_step.argtypes = [vp, i32]
         L.ccake_synchronize.argtypes = [vp]
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
@@ -209,6 +211,26 @@ class Ccake:
         self._chk(lib().ccake_smear_sources(self._h, t.size, pp, rr, t.ctypes.data, float(h_source), float(eta_norm),
                                             oo, HOST), "ccake_smear_sources")
         return out
+
+    def set_sources(self, I=None, Iq=None):
+        """ccake_set_sources (Eq. 38): I [4, n] contravariant I^mu, Iq [3, n] (numpy host arrays, or lists of
+        CUDA tensors of n doubles); None = zero; both None switches the sources off."""
+        keep = []
+        space = HOST
+
+        def ptrs(a, k):
+            nonlocal space
+            if a is None:
+                return None
+            if _is_torch(a[0]):
+                space = DEVICE
+                keep.extend(a)
+                return (C.c_void_p * k)(*[t.data_ptr() for t in a])
+            a = np.ascontiguousarray(a, dtype=np.float64).reshape(k, self.n)
+            keep.append(a)
+            return (C.c_void_p * k)(*[a[m].ctypes.data for m in range(k)])
+        pi, pq = ptrs(I, 4), ptrs(Iq, 3)
+        self._chk(lib().ccake_set_sources(self._h, pi, pq, space), "ccake_set_sources")
 
     def step(self, nsteps=1):
         self._chk(lib().ccake_step(self._h, nsteps), "ccake_step")

@@ -60,6 +60,8 @@ struct ccake_ctx {
   uint32_t* nnb = nullptr;
   double* theta = nullptr;
   double* scratch = nullptr;    /* N doubles: read_fields staging */
+  double* src = nullptr;        /* 7 x npad, original order: I^mu, I_q of ccake_set_sources (allocated on first use) */
+  bool has_src = false;
   Sorted so;
 
   TableDev tb;
@@ -111,6 +113,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->nnb); c->nnb = nullptr;
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
+  cudaFree(c->src); c->src = nullptr; c->has_src = false;
   c->loaded = false;
 }
 
@@ -238,6 +241,8 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   RkArgs rk = rk_in;
   rk.Ycur = Ycur;
   rk.theta_out = c->theta;
+  rk.src = c->has_src ? c->src : nullptr;
+  rk.orig = c->orig[0];
   if (rk.diag) eom_kernel<D, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
   else eom_kernel<D, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
   if ((rc = mark(c))) return rc;
@@ -644,6 +649,7 @@ static int reload_particles(ccake_ctx* c, int32_t nfields, const int32_t* ids, c
   c->launches += 2;
   c->x0 = c->P.x0_start;
   c->derived_valid = false;
+  c->has_src = false;
   return launch_check(c, "reload");
 }
 
@@ -898,6 +904,28 @@ int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4]
   cudaFree(dsrc);
   cudaFree(dout);
   return rc;
+}
+
+int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* const Iq[3], int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (memspace != 0 && memspace != 1) { c->err = "bad memspace"; return CCAKE_EINVAL; }
+  if (!c->loaded) { c->err = "sources before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  bool any = false;
+  for (int m = 0; m < 7; ++m) any = any || ((m < 4) ? (I && I[m]) : (Iq && Iq[m - 4]));
+  c->derived_valid = false;
+  if (!any) { c->has_src = false; return CCAKE_OK; }
+  const int64_t np = c->npad, n = c->N;
+  if (!c->src) CK(cudaMalloc(&c->src, sizeof(double) * 7 * np));
+  CK(cudaMemsetAsync(c->src, 0, sizeof(double) * 7 * np, c->stream));
+  const cudaMemcpyKind kind = (memspace == CCAKE_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  for (int m = 0; m < 7; ++m) {
+    const double* col = (m < 4) ? (I ? I[m] : nullptr) : (Iq ? Iq[m - 4] : nullptr);
+    if (col) CK(cudaMemcpyAsync(c->src + (int64_t)m * np, col, sizeof(double) * n, kind, c->stream));
+  }
+  if (memspace == CCAKE_HOST) CK(cudaStreamSynchronize(c->stream));      /* the caller may reuse its buffers */
+  c->has_src = true;
+  return CCAKE_OK;
 }
 
 int ccake_step(ccake_ctx* c, int32_t nsteps) {

@@ -38,7 +38,8 @@ struct EomIn {
   double thc;            /* gamma (div v + Gamma_g) */
   double rhsJ[NQ][3];    /* constant right-hand side of the diffusion equation */
   double FM[3];          /* sqrt(-g) (FP_i - FB_i) */
-  double FKs[NQ];        /* sqrt(-g) FK_q */
+  double FKs[NQ];        /* sqrt(-g) FK_q - I_q / (gamma sigma) */
+  double uI;             /* u_mu I^mu, source of the entropy equation (Eq. 96); 0 without sources */
   Dissip ds;
 };
 
@@ -214,7 +215,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
     o.dN[q] = -in.FKs[q] - o.dJt[q][0] * igam + (in.ds.Jt[q][0] * (igam * igam)) * du[0];
   /* entropy, Eq. 96: gamma sigma (T dS + mu_q dN_q) = -Pi theta + pi^mu_nu nabla_mu u^nu */
   {
-    double rhs = -Pi * theta;
+    double rhs = -Pi * theta + in.uI;
     if (kp.shear)
 #pragma unroll
       for (int m = 0; m < 4; ++m)
@@ -252,6 +253,8 @@ struct RkArgs {
   double* Krate;        /* rates in store order, or NULL           */
   double* theta_out;    /* sorted order                            */
   double* diag;         /* 4 x npad, sorted order: Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1 (DIAG kernels only) */
+  const double* src;    /* 7 x npad, ORIGINAL particle order: I^0..I^3, I_B, I_S, I_Q (ccake_set_sources), or NULL */
+  const uint32_t* orig; /* store slot -> original index (for src)  */
   double c_out, w_acc;
   int acc_mode;         /* 0 none | 1 set | 2 add | 3 final        */
   int update;           /* 0: rates only (refresh)                 */
@@ -359,6 +362,22 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   for (int k = 0; k < 3; ++k) in.FM[k] = (k < D) ? gm.sqrtg * (so.FP[k][i] - so.FB[k][i]) : 0.0;
 #pragma unroll
   for (int q = 0; q < NQ; ++q) in.FKs[q] = gm.sqrtg * so.FK[q][i];
+  in.uI = 0.0;
+  if (rk.src) {
+    /* source terms, Eq. 38 (:623), Eq. 42-44 (:645-649), Eq. 96 (:1003):
+         d/dx0 [C u_i + pi~^0_i / gamma] += I_i / (gamma sigma),  d/dx0 [N_q + J~^0_q / gamma] += I_q / (gamma sigma),
+         gamma sigma (T dS + mu_q dN_q)  += u_mu I^mu */
+    const int64_t oid = rk.orig[a];
+    const double igs = in.igam * in.isig;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      const double Im = (m <= D) ? rk.src[m * npad + oid] : 0.0;
+      in.uI += in.ulo[m] * Im;
+      if (m >= 1 && m <= D) in.FM[m - 1] += in.glo[m] * Im * igs;
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) in.FKs[q] -= rk.src[(4 + q) * npad + oid] * igs;
+  }
   if (kp.diff) {
     /* tau_q sigma [...] = -J^i_q + sum_q' kappa_qq' nabla^<i> alpha_q',  nabla^<i> alpha = g^{ii} d_i alpha - u^i u^j d_j alpha */
     double udota[NQ];

@@ -48,3 +48,47 @@ def test_source_smearing_matches_oracle(name, steps):
     z = g.smear_sources(np.zeros((4, 0)), np.zeros((3, 0)), np.zeros(0), 1.4, 0.62)
     assert np.all(z == 0.0)
     g.close()
+
+
+@pytest.mark.parametrize("name", ["C1", "C1h", "C4_small", "C3_small", "cloud3_hyp_dnmr_rk4"])
+def test_sources_in_the_equations_of_motion(name):
+    """Rest of NEXT-3, Eq. 38 / 42-44 / 96: 1,500 partons per step smeared onto the particles (Eq. 35), fed
+    back as I^mu together with seeded charge sources I_q, for 4 steps (dynamical initialisation: new partons every
+    step).  Rates at the first step 1e-10 of the field norm, every evolved field 1e-8 after the run; switching the
+    sources off restores the source-free rates bit by bit."""
+    from test_gpu_parity import WORKLOADS
+    from gpu_common import TOL_GRAD, TOL_RUN, assert_fields, state_ids
+    w = WORKLOADS[name]()
+    g, o = make_pair(w)
+    D = w.params["dim"]
+    dx0 = w.params["dx0"]
+    ext = float(np.max(np.abs(w.fields[B.R1]))) * 0.6
+    rate_ids = [B.RATE + k for k in state_ids(w.params)]
+    free = g.read_fields(rate_ids)
+    rng = np.random.default_rng(96)
+    scale = float(np.mean(w.fields[B.S])) * 0.02
+    for step in range(4):
+        x0 = w.params["x0_start"] + step * dx0
+        p, r, t = _partons(rng, 1500, D, ext, x0, dx0)
+        jg = g.smear_sources(p * scale, r, t, 1.4, 0.62)
+        jo = o.smear_sources(p * scale, r, t, 1.4, 0.62)
+        iq = 0.01 * scale * rng.normal(0.0, 1.0, (3, w.n)) * np.abs(jo[0]) / max(np.abs(jo[0]).max(), 1e-300)
+        g.set_sources(jg, iq)
+        o.set_sources(jo, iq)
+        if step == 0:
+            assert_fields(g, o, rate_ids, TOL_GRAD, name + " rates with sources")
+            with_src = g.read_fields(rate_ids)
+            assert any(np.max(np.abs(with_src[k] - free[k])) > 0 for k in rate_ids)
+        g.step(1)
+        o.step(1)
+    g.synchronize(strict=False)
+    assert_fields(g, o, state_ids(w.params), TOL_RUN, name + " state after 4 steps with sources")
+    g.close()
+    # off again: identical to a context that never had sources
+    g1 = B.from_workload(w)
+    g1.set_sources(np.ones((4, w.n)), None)
+    g1.set_sources(None, None)
+    again = g1.read_fields(rate_ids)
+    for k in rate_ids:
+        assert np.array_equal(again[k], free[k])
+    g1.close()
