@@ -219,3 +219,29 @@ def eos_forward(params: Params, T, mu):
     if rc:
         raise OracleError(f"oracle_eos_forward rc={rc}")
     return np.array(out[:])
+
+
+def invert_forward_table(params: Params, faxes, fdata, s, n):
+    """oracle_invert_forward_table: faxes = 4 increasing axes (T, mu_B, mu_S, mu_Q), fdata[..., 5] = (p, s, n_B, n_S, n_Q) at
+    the nodes, targets s[a], n[q][a].  Returns (out[nt, 11], flag[nt], iters[nt])."""
+    faxes = [np.ascontiguousarray(a, dtype=np.float64) for a in faxes]
+    fdata = np.ascontiguousarray(fdata, dtype=np.float64)
+    dims = (C.c_int32 * 4)(*[len(a) for a in faxes])
+    assert fdata.size == int(np.prod([len(a) for a in faxes])) * 5
+    ax = (C.POINTER(C.c_double) * 4)(*[a.ctypes.data_as(C.POINTER(C.c_double)) for a in faxes])
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    nn = [np.ascontiguousarray(n[q], dtype=np.float64) for q in range(3)]
+    nt = s.size
+    npt = (C.POINTER(C.c_double) * 3)(*[a.ctypes.data_as(C.POINTER(C.c_double)) for a in nn])
+    out = np.zeros((nt, 11))
+    flag = np.zeros(nt, dtype=np.int32)
+    iters = np.zeros(nt, dtype=np.int32)
+    L = lib()
+    L.oracle_invert_forward_table.restype = C.c_int
+    L.oracle_invert_forward_table.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p,
+                                              C.c_void_p, C.c_void_p, C.c_void_p]
+    rc = L.oracle_invert_forward_table(C.byref(params), dims, ax, fdata.ctypes.data, nt, s.ctypes.data, npt,
+                                       out.ctypes.data, flag.ctypes.data, iters.ctypes.data)
+    if rc:
+        raise OracleError(f"oracle_invert_forward_table rc={rc}")
+    return out, flag, iters

@@ -461,6 +461,156 @@ static Thermo eos_table(const Table& tb, double s, const double n[NQ]) {
   return th;
 }
 
+/* ------------------------------------------------ offline inverter on a tabulated forward EoS (:576-593) ---- */
+/* PAPER.md :583 ("takes a given EoS on a fixed grid of {T, mu} coupled with the backup EoS and then converts this to a
+   single EoS table on a fixed grid in {s, n}"), :587 ("the offline inversion procedure uses the existing root-finder and
+   interpolator").  The paper prints neither; DESIGN reading 21 fixes them, and this follows it step by step:
+     interpolator   quadrilinear blend of the forward columns (p, s, n_B, n_S, n_Q) at X = (T, mu_B, mu_S, mu_Q), X clamped
+                    to the grid box; the Jacobian J_ik = d(s, n)_i / dX_k is the derivative of that blend inside its cell
+     start          mu_q = 0 (clamped to the axis), T by 60 bisections of s(T, mu) = s* over the T axis
+     root-finder    damped Newton, at most 40 iterations: converged when max_i |Y_i - Y*_i| <= 1e-13 s*; J delta = -(Y - Y*)
+                    by dense elimination; lambda = 1, 1/2, ... (at most 12 halvings) until the squared residual decreases
+     result         T, mu = X; p = blend; e = T s* - p + mu_q n*_q (Euler relation); z = J^-T Y*: dw/ds = T + z_0,
+                    dw/dn_q = mu_q + z_q (chain rule on w = T s + mu_q n_q); c_s^2 = (Y* . J^-1 Y*) / (X . Y*), i.e. dp/de
+                    along fixed n_q / s (dp = Y . dX, de = X . dY)
+     backup EoS     a target the root-finder does not reach (singular J, no decrease, iterations used up) takes the
+                    closed-form conformal EoS of the parameters (:572: "progressively moves on to the next EoS"), flag 1 */
+struct FwdTable {
+  int32_t dims[4];
+  const double* ax[4];
+  const double* data;      /* [node][5]: p, s, n_B, n_S, n_Q; node = ((i0 * d1 + i1) * d2 + i2) * d3 + i3 */
+};
+
+static void fwd_interp(const FwdTable& ft, const double Xin[4], double Y[5], double J[16]) {
+  int i0[4];
+  double t[4], w[4];
+  for (int k = 0; k < 4; ++k) {
+    const double* ax = ft.ax[k];
+    const int nn = ft.dims[k];
+    double xv = Xin[k];
+    if (!(xv >= ax[0])) xv = ax[0];
+    if (!(xv <= ax[nn - 1])) xv = ax[nn - 1];
+    int i = (int)(std::upper_bound(ax, ax + nn, xv) - ax) - 1;
+    if (i > nn - 2) i = nn - 2;
+    if (i < 0) i = 0;
+    i0[k] = i;
+    w[k] = ax[i + 1] - ax[i];
+    t[k] = (xv - ax[i]) / w[k];
+  }
+  for (int c = 0; c < 5; ++c) Y[c] = 0.0;
+  for (int k = 0; k < 16; ++k) J[k] = 0.0;
+  for (int corner = 0; corner < 16; ++corner) {
+    int b[4];
+    for (int k = 0; k < 4; ++k) b[k] = (corner >> (3 - k)) & 1;
+    const int64_t node = (((int64_t)(i0[0] + b[0]) * ft.dims[1] + (i0[1] + b[1])) * ft.dims[2] + (i0[2] + b[2])) * ft.dims[3] + (i0[3] + b[3]);
+    const double* f = ft.data + node * 5;
+    double wk[4];
+    for (int k = 0; k < 4; ++k) wk[k] = b[k] ? t[k] : 1.0 - t[k];
+    const double wall = ((wk[0] * wk[1]) * wk[2]) * wk[3];
+    for (int c = 0; c < 5; ++c) Y[c] += wall * f[c];
+    for (int k = 0; k < 4; ++k) {
+      /* d/dX_k of the blend: the weight of axis k is replaced by -+ 1 / (cell width) */
+      double wd = (b[k] ? 1.0 : -1.0) / w[k];
+      for (int m = 0; m < 4; ++m) if (m != k) wd *= wk[m];
+      for (int i = 0; i < 4; ++i) J[i * 4 + k] += wd * f[1 + i];
+    }
+  }
+}
+
+static Thermo invert_forward_point(const oracle_params& P, const FwdTable& ft, double s, const double n[NQ], int32_t& flag,
+                                   int32_t& iters) {
+  const double Ys[4] = {s, n[0], n[1], n[2]};
+  double X[4], Y[5], J[16];
+  auto clampX = [&](double* x) {
+    for (int k = 0; k < 4; ++k) {
+      if (!(x[k] >= ft.ax[k][0])) x[k] = ft.ax[k][0];
+      if (!(x[k] <= ft.ax[k][ft.dims[k] - 1])) x[k] = ft.ax[k][ft.dims[k] - 1];
+    }
+  };
+  auto res2 = [&](const double* y) {
+    double r = 0.0;
+    for (int i = 0; i < 4; ++i) { const double d = (y[1 + i] - Ys[i]) / s; r += d * d; }
+    return r;
+  };
+  /* start */
+  X[0] = 0.0; X[1] = X[2] = X[3] = 0.0;
+  clampX(X);
+  {
+    double lo = ft.ax[0][0], hi = ft.ax[0][ft.dims[0] - 1];
+    for (int it = 0; it < 60; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      X[0] = mid;
+      fwd_interp(ft, X, Y, J);
+      if (Y[1] > s) hi = mid; else lo = mid;
+    }
+    X[0] = 0.5 * (lo + hi);
+  }
+  fwd_interp(ft, X, Y, J);
+  bool ok = false;
+  iters = 0;
+  for (int it = 0; it < 40; ++it) {
+    double rmax = 0.0;
+    for (int i = 0; i < 4; ++i) rmax = std::max(rmax, std::fabs(Y[1 + i] - Ys[i]));
+    if (rmax <= 1e-13 * s) { ok = true; break; }
+    double A[16], d[4];
+    for (int k = 0; k < 16; ++k) A[k] = J[k];
+    for (int i = 0; i < 4; ++i) d[i] = -(Y[1 + i] - Ys[i]);
+    if (!dense_solve(4, A, d)) break;
+    const double r0 = res2(Y);
+    double lam = 1.0;
+    bool acc = false;
+    for (int hv = 0; hv <= 12; ++hv) {
+      double Xn[4], Yn[5], Jn[16];
+      for (int k = 0; k < 4; ++k) Xn[k] = X[k] + lam * d[k];
+      clampX(Xn);
+      fwd_interp(ft, Xn, Yn, Jn);
+      if (res2(Yn) < r0) {
+        for (int k = 0; k < 4; ++k) X[k] = Xn[k];
+        for (int c = 0; c < 5; ++c) Y[c] = Yn[c];
+        for (int k = 0; k < 16; ++k) J[k] = Jn[k];
+        acc = true;
+        break;
+      }
+      lam *= 0.5;
+    }
+    ++iters;
+    if (!acc) break;
+  }
+  if (!ok) {
+    double rmax = 0.0;
+    for (int i = 0; i < 4; ++i) rmax = std::max(rmax, std::fabs(Y[1 + i] - Ys[i]));
+    ok = rmax <= 1e-13 * s;
+  }
+  Thermo th;
+  std::memset(&th, 0, sizeof(th));
+  double A[16], z[4], v[4];
+  if (ok) {
+    for (int i = 0; i < 4; ++i) for (int k = 0; k < 4; ++k) A[i * 4 + k] = J[k * 4 + i];     /* J^T */
+    for (int i = 0; i < 4; ++i) z[i] = Ys[i];
+    ok = dense_solve(4, A, z);
+  }
+  if (ok) {
+    for (int k = 0; k < 16; ++k) A[k] = J[k];
+    for (int i = 0; i < 4; ++i) v[i] = Ys[i];
+    ok = dense_solve(4, A, v);
+  }
+  if (!ok) {
+    flag = 1;
+    return eos_closed_form(P, s, n);
+  }
+  flag = 0;
+  th.T = X[0];
+  for (int q = 0; q < NQ; ++q) th.mu[q] = X[1 + q];
+  th.p = Y[0];
+  th.e = X[0] * s - Y[0] + (X[1] * n[0] + X[2] * n[1] + X[3] * n[2]);
+  th.ws = X[0] + z[0];
+  for (int q = 0; q < NQ; ++q) th.wq[q] = X[1 + q] + z[1 + q];
+  double num = 0.0, den = 0.0;
+  for (int i = 0; i < 4; ++i) { num += Ys[i] * v[i]; den += X[i] * Ys[i]; }
+  th.cs2 = num / den;
+  return th;
+}
+
 /* transport coefficients, §5.3 :732-769 and DESIGN reading 11 */
 struct Transport { double eta, zeta, tau_pi, tau_Pi, kappa[NQ][NQ], tau_q[NQ]; };
 
@@ -1357,6 +1507,29 @@ int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double o
   const Thermo th = eos_table(c->tab, s, n);
   thermo_to_out(th, out);
   if (oob) *oob = th.oob;
+  return ORACLE_OK;
+}
+
+int oracle_invert_forward_table(const oracle_params* p, const int32_t fdims[4], const double* const faxes[4], const double* fdata,
+                                int64_t nt, const double* s, const double* const n[3], double* out, int32_t* flag, int32_t* iters) {
+  if (!p || !fdims || !faxes || !fdata || nt < 0 || !s || !n || !out || !flag) return ORACLE_EINVAL;
+  FwdTable ft;
+  for (int k = 0; k < 4; ++k) {
+    if (fdims[k] < 2 || !faxes[k]) return ORACLE_EINVAL;
+    for (int i = 1; i < fdims[k]; ++i) if (!(faxes[k][i] > faxes[k][i - 1])) return ORACLE_EINVAL;
+    ft.dims[k] = fdims[k];
+    ft.ax[k] = faxes[k];
+  }
+  ft.data = fdata;
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t a = 0; a < nt; ++a) {
+    const double nn[NQ] = {n[0][a], n[1][a], n[2][a]};
+    int32_t f = 0, it = 0;
+    const Thermo th = invert_forward_point(*p, ft, s[a], nn, f, it);
+    thermo_to_out(th, out + a * 11);
+    flag[a] = f;
+    if (iters) iters[a] = it;
+  }
   return ORACLE_OK;
 }
 

@@ -86,6 +86,14 @@ int oracle_eos_closed_form(const oracle_params* p, double s, const double n[3], 
 int oracle_eos_forward(const oracle_params* p, double T, const double mu[3], double out[5]);
 int oracle_eos_table_lookup(oracle_ctx* c, double s, const double n[3], double out[11], int32_t* oob);
 
+/* Offline inverter on a TABULATED forward EoS (PAPER.md :576-593; DESIGN reading 21): fdata holds (p, s, n_B, n_S, n_Q) at
+ * the nodes of the (T, mu_B, mu_S, mu_Q) grid faxes (strictly increasing, fdims nodes each, last axis fastest).  For each
+ * of the nt targets (s[a], n[q][a]): damped 4-D Newton on the quadrilinear interpolant; out[a*11 .. a*11+10] = T, mu_B,
+ * mu_S, mu_Q, p, c_s^2, e, dw/ds, dw/dn_B, dw/dn_S, dw/dn_Q; flag[a] = 0 (found in the table) or 1 (the backup EoS,
+ * the closed-form conformal one of *p, was used); iters (may be NULL) = Newton iterations taken. */
+int oracle_invert_forward_table(const oracle_params* p, const int32_t fdims[4], const double* const faxes[4], const double* fdata,
+                                int64_t nt, const double* s, const double* const n[3], double* out, int32_t* flag, int32_t* iters);
+
 /* Source smearing of PAPER.md Eq. 35 (:521), the gather half of the dynamical initialisation: for every loaded
  * particle i,  j^mu_i = eta_norm / (dx0 sqrt(-g)) * sum over partons k with x0 - dx0 < t_k <= x0 of
  * p^mu_k W(r_i - r_k; h_source), W the cubic spline of Eq. 77 in the context's dimension, x0 the current time and
