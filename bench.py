@@ -381,6 +381,23 @@ def run_ours(args):
         t_cpu = time.perf_counter() - t0
         eos_inv = {"nodes": nodes, "columns": len(tb["col_ids"]), "gpu_ms": 1e3 * t_gpu, "gpu_nodes_per_s": nodes / t_gpu,
                    "cpu_oracle_nodes_per_s": nsample / t_cpu, "cpu_sample": f"{nsample} seeded nodes, 1 thread, through ctypes"}
+        # rest of NEXT-1: the same target grid from a TABULATED forward EoS (BASELINE.json configs[1]: 100 x 32^3 (T, mu) grid),
+        # damped 4-D Newton per node on the device; the oracle's inverter on a seeded sample of nodes beside it
+        ft = W.make_forward_table(100, 32)
+        sim.invert_forward_table(ft["axes"], ft["data"], tb["axes"], tb["axis_kind"], tb["col_ids"])      # warm-up
+        t0 = time.perf_counter()
+        _, _, n_backup = sim.invert_forward_table(ft["axes"], ft["data"], tb["axes"], tb["axis_kind"], tb["col_ids"])
+        t_fwd = time.perf_counter() - t0
+        sv = tb["axes"][0][ii[0]]
+        nv = [tb["axes"][q + 1][ii[q + 1]] * sv for q in range(3)]
+        t0 = time.perf_counter()
+        O.invert_forward_table(P, ft["axes"], ft["data"], sv, nv)
+        t_cpu_fwd = time.perf_counter() - t0
+        eos_inv["forward_table"] = {"forward_grid": [len(a) for a in ft["axes"]], "gpu_ms": 1e3 * t_fwd,
+                                    "gpu_nodes_per_s": nodes / t_fwd, "nodes_on_backup_eos": n_backup,
+                                    "cpu_oracle_nodes_per_s": nsample / t_cpu_fwd,
+                                    "cpu_sample": f"{nsample} seeded nodes, OpenMP over nodes, {os.cpu_count()} cores",
+                                    "note": "gpu_ms includes the 131 MB host-to-device copy of the forward table"}
         sim.load_eos_table(tb["axes"], tb["axis_kind"], tb["col_ids"], torch.as_tensor(tb["data"], device=dev))
 
     # ---- NEXT-2: freeze-out element pass (one more pair pass over the cached lists and masks), device buffers ----

@@ -126,10 +126,24 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
  * solves (T, mu_q) from (s, n_q) — the cubic of Eq. A.13-A.14 for mu_q(T) inside a bisection in T on the monotone
  * s(T, mu(T)) — evaluates p, e = 3p, c_s^2 = 1/3, dw/ds and dw/dn_q there, and installs the result as the
  * context's table exactly as ccake_load_eos_table would.  out may be NULL; otherwise it receives the table,
- * [d0][d1][d2][d3][ncols] doubles.  Other equations of state are inverted elsewhere and loaded. */
+ * [d0][d1][d2][d3][ncols] doubles.  A tabulated equation of state goes through ccake_invert_forward_table. */
 int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4],
                            const double* const axes[4], int32_t ncols, const int32_t* col_ids, double* out,
                            int32_t memspace);
+
+/* Rest of NEXT-1: the offline inverter on a TABULATED forward EoS (PAPER.md :576-593, footnote :585; DESIGN reading 21).
+ * fdata holds (p, s, n_B, n_S, n_Q) — 5 doubles per node — on the (T, mu_B, mu_S, mu_Q) grid faxes (fdims nodes per
+ * axis, strictly increasing, any spacing; row-major, last axis fastest).  For every node (s*, n*_q) of the target grid
+ * dims / axis_kind / axes (as in ccake_load_eos_table) one device thread solves interp(T, mu) = (s*, n*) by damped
+ * Newton on the quadrilinear interpolant — start: mu = 0, T by bisection on s; at most 40 iterations, converged at
+ * max |residual| <= 1e-13 s*; step halving until the residual decreases — and writes T, mu_q, p = interp, e = T s* - p +
+ * mu_q n*_q, dw/ds, dw/dn_q and c_s^2 from the interpolant's Jacobian.  A node the root-finder does not reach takes the
+ * backup EoS (:572): the closed-form conformal family of params, flag 1.  The result is installed as the context's
+ * table; out ([d0][d1][d2][d3][ncols] doubles), flags (one int32 per node: 0 table, 1 backup) may be NULL; n_backup
+ * (host, may be NULL) receives the number of flagged nodes.  faxes[k], fdata, axes[k], out, flags live in `memspace`. */
+int ccake_invert_forward_table(ccake_ctx* c, const int32_t fdims[4], const double* const faxes[4], const double* fdata,
+                               const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4], int32_t ncols,
+                               const int32_t* col_ids, double* out, int32_t* flags, int64_t* n_backup, int32_t memspace);
 
 /* NEXT-3 (part) of SURVEY.md §8(f): the source smearing of PAPER.md Eq. 35 (:521), the gather half of the dynamical
  * initialisation.  For every loaded particle i, at the context's current time x0 and step dx0,

@@ -30,7 +30,7 @@ RATE = 64
 HOST, DEVICE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_smear_sources",
+EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_invert_forward_table", "ccake_smear_sources",
            "ccake_set_sources",
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
@@ -75,6 +75,8 @@ def lib():
         L.ccake_load_particles.argtypes = [vp, i64, i32, C.POINTER(i32), C.POINTER(vp), i32]
         L.ccake_load_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
         L.ccake_invert_eos_table.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(i32), vp, i32]
+        L.ccake_invert_forward_table.argtypes = [vp, C.POINTER(i32), C.POINTER(vp), vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32,
+                                                 C.POINTER(i32), vp, vp, C.POINTER(i64), i32]
         L.ccake_smear_sources.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp), i32]
         L.ccake_set_sources.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), i32]
         L.ccake_step.argtypes = [vp, i32]
@@ -199,6 +201,27 @@ class Ccake:
         self._chk(lib().ccake_invert_eos_table(self._h, dims, kinds, ptrs, len(col_ids), cids,
                                                res.ctypes.data if out else None, HOST), "ccake_invert_eos_table")
         return res
+
+    def invert_forward_table(self, faxes, fdata, axes, axis_kind, col_ids, out=False):
+        """ccake_invert_forward_table: invert the forward table fdata[..., 5] = (p, s, n_B, n_S, n_Q) on the (T, mu) grid
+        faxes onto the (s, B, S, Q) grid axes on the device and install it.  Returns (table or None, flags, n_backup)."""
+        fax = [np.ascontiguousarray(a, dtype=np.float64) for a in faxes]
+        fdata = np.ascontiguousarray(fdata, dtype=np.float64)
+        assert fdata.size == int(np.prod([len(a) for a in fax])) * 5
+        ax = [np.ascontiguousarray(a, dtype=np.float64) for a in axes]
+        fdims = (C.c_int32 * 4)(*[len(a) for a in fax])
+        dims = (C.c_int32 * 4)(*[len(a) for a in ax])
+        kinds = (C.c_int32 * 4)(*axis_kind)
+        cids = (C.c_int32 * len(col_ids))(*col_ids)
+        fptrs = (C.c_void_p * 4)(*[a.ctypes.data for a in fax])
+        ptrs = (C.c_void_p * 4)(*[a.ctypes.data for a in ax])
+        res = np.empty([len(a) for a in ax] + [len(col_ids)], dtype=np.float64) if out else None
+        flags = np.zeros([len(a) for a in ax], dtype=np.int32)
+        nb = C.c_int64(0)
+        self._chk(lib().ccake_invert_forward_table(self._h, fdims, fptrs, fdata.ctypes.data, dims, kinds, ptrs, len(col_ids), cids,
+                                                   res.ctypes.data if out else None, flags.ctypes.data, C.byref(nb), HOST),
+                  "ccake_invert_forward_table")
+        return res, flags, int(nb.value)
 
     def smear_sources(self, p, r, t, h_source, eta_norm=1.0):
         """ccake_smear_sources (Eq. 35): p [4, np], r [3, np], t [np] (numpy, host) -> j [4, n] numpy."""

@@ -864,6 +864,92 @@ int ccake_invert_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t ax
   return rc;
 }
 
+int ccake_invert_forward_table(ccake_ctx* c, const int32_t fdims[4], const double* const faxes[4], const double* fdata,
+                               const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4], int32_t ncols,
+                               const int32_t* col_ids, double* out, int32_t* flags, int64_t* n_backup, int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (!fdims || !faxes || !fdata || !dims || !axis_kind || !axes || !col_ids || ncols <= 0 || ncols > CCAKE_NCOLS_MAX ||
+      (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_invert_forward_table";
+    return CCAKE_EINVAL;
+  }
+  int64_t nodes = 1, nax = 0, fnodes = 1, fnax = 0;
+  for (int k = 0; k < 4; ++k) {
+    if (dims[k] < 2 || !axes[k] || (axis_kind[k] != 0 && axis_kind[k] != 1) || (k == 0 && axis_kind[k] != 0) || fdims[k] < 2 ||
+        !faxes[k]) {
+      c->err = "bad table axis";
+      return CCAKE_EINVAL;
+    }
+    nodes *= dims[k]; nax += dims[k];
+    fnodes *= fdims[k]; fnax += fdims[k];
+  }
+  InvertArgs ia;
+  std::memset(&ia, 0, sizeof(ia));
+  for (int cc = 0; cc < CCAKE_NCOLS_MAX; ++cc) ia.col_of[cc] = -1;
+  for (int k = 0; k < ncols; ++k) {
+    if (col_ids[k] < 0 || col_ids[k] >= CCAKE_NCOLS_MAX) { c->err = "bad column id"; return CCAKE_EINVAL; }
+    ia.col_of[col_ids[k]] = k;
+  }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  const cudaMemcpyKind in = (memspace == CCAKE_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const cudaMemcpyKind outk = (memspace == CCAKE_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+  /* the forward axes must be strictly increasing: checked on a host copy */
+  std::vector<double> hfax(fnax);
+  {
+    int64_t off = 0;
+    for (int k = 0; k < 4; ++k) {
+      CK(cudaMemcpy(hfax.data() + off, faxes[k], sizeof(double) * fdims[k], memspace == CCAKE_HOST ? cudaMemcpyHostToHost : cudaMemcpyDeviceToHost));
+      for (int i = 1; i < fdims[k]; ++i)
+        if (!(hfax[off + i] > hfax[off + i - 1])) { c->err = "forward axis not increasing"; return CCAKE_EINVAL; }
+      off += fdims[k];
+    }
+  }
+  /* one allocation: target axes | forward axes | forward data (when it comes from the host) | inverted table | flags | counter */
+  const bool copy_fdata = memspace == CCAKE_HOST;
+  const size_t n_dbl = (size_t)nax + (size_t)fnax + (copy_fdata ? (size_t)fnodes * 5 : 0) + (size_t)nodes * ncols + 1;
+  double* buf = nullptr;
+  int* dflags = nullptr;
+  if (cudaMalloc(&buf, sizeof(double) * n_dbl) != cudaSuccess) { cudaGetLastError(); c->err = "inverter buffers"; return CCAKE_ENOMEM; }
+  if (cudaMalloc(&dflags, sizeof(int) * nodes) != cudaSuccess) { cudaGetLastError(); cudaFree(buf); c->err = "inverter buffers"; return CCAKE_ENOMEM; }
+  double* dax = buf;
+  double* dfax = dax + nax;
+  double* dfdata = dfax + fnax;
+  double* ddata = dfdata + (copy_fdata ? fnodes * 5 : 0);
+  unsigned long long* dcount = reinterpret_cast<unsigned long long*>(ddata + nodes * ncols);
+  cudaStream_t st = c->stream;
+  FwdDev fd;
+  const double* daxes[4];
+  {
+    int64_t off = 0, foff = 0;
+    for (int k = 0; k < 4; ++k) {
+      cudaMemcpyAsync(dax + off, axes[k], sizeof(double) * dims[k], in, st);
+      ia.dims[k] = dims[k]; ia.kind[k] = axis_kind[k]; ia.ax[k] = dax + off; daxes[k] = dax + off;
+      off += dims[k];
+      fd.dims[k] = fdims[k]; fd.ax[k] = dfax + foff;
+      foff += fdims[k];
+    }
+  }
+  cudaMemcpyAsync(dfax, hfax.data(), sizeof(double) * fnax, cudaMemcpyHostToDevice, st);
+  if (copy_fdata) cudaMemcpyAsync(dfdata, fdata, sizeof(double) * fnodes * 5, cudaMemcpyHostToDevice, st);
+  fd.data = copy_fdata ? dfdata : fdata;
+  cudaMemsetAsync(dcount, 0, sizeof(unsigned long long), st);
+  ia.ncols = ncols;
+  eos_invert_fwd_kernel<<<nblk(nodes, 128), 128, 0, st>>>(c->kp, ia, fd, nodes, ddata, dflags, dcount);
+  c->launches += 1;
+  int rc = launch_check(c, "eos_invert_fwd_kernel");
+  unsigned long long nb = 0;
+  if (rc == CCAKE_OK && (cudaMemcpyAsync(&nb, dcount, sizeof(nb), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                         cudaStreamSynchronize(st) != cudaSuccess)) { c->err = "eos_invert_fwd_kernel failed"; rc = CCAKE_ECUDA; }
+  if (rc == CCAKE_OK) rc = ccake_load_eos_table(c, dims, axis_kind, daxes, ncols, col_ids, ddata, CCAKE_DEVICE);
+  if (rc == CCAKE_OK && out && cudaMemcpy(out, ddata, sizeof(double) * nodes * ncols, outk) != cudaSuccess) { c->err = "copy of the inverted table"; rc = CCAKE_ECUDA; }
+  if (rc == CCAKE_OK && flags && cudaMemcpy(flags, dflags, sizeof(int) * nodes, outk) != cudaSuccess) { c->err = "copy of the flags"; rc = CCAKE_ECUDA; }
+  if (n_backup) *n_backup = (int64_t)nb;
+  cudaFree(buf);
+  cudaFree(dflags);
+  return rc;
+}
+
 int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3], const double* t,
                         double h_source, double eta_norm, double* const j[4], int32_t memspace) {
   if (!c) return CCAKE_EINVAL;

@@ -47,30 +47,36 @@ struct EomOut {
   double du0, theta, dS, dN[NQ], dBulk, dpit[4][4], dJt[NQ][4], res[3];
 };
 
-template <int D>
+/* MODE 0: the rates at a given du.  MODE 1: at du = 0 (a literal, so every du term folds away).  MODE 2 + c: the
+   HOMOGENEOUS part of the affine map at the unit vector e_c — every term without du is dropped (K = 0 below) and the
+   zeros of e_c fold away, so res is column c of the matrix of Eq. 95 directly (no difference of two evaluations). */
+template <int D, int MODE>
 __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, const EomIn& in, const double du_in[3],
                                           EomOut& o, double* sgsq_out = nullptr) {
+  constexpr bool H = MODE >= 2;
+  constexpr double K = H ? 0.0 : 1.0;            /* multiplies the du-independent terms */
   const double gam = in.gam, sig = in.sig;
   const double igam = in.igam, itau = in.itau;
   double du[4], dulo[4];
-  du[1] = du_in[0]; du[2] = du_in[1]; du[3] = (D == 3) ? du_in[2] : 0.0;
+  if (MODE == 0) { du[1] = du_in[0]; du[2] = du_in[1]; du[3] = (D == 3) ? du_in[2] : 0.0; }
+  else { du[1] = (MODE == 2) ? 1.0 : 0.0; du[2] = (MODE == 3) ? 1.0 : 0.0; du[3] = (MODE == 4) ? 1.0 : 0.0; }
   /* Eq. 97, nu = 0: u_0 du^0 = -u_k du^k - (1/2) u^a u^b dg_ab/dx0,  dg_33/dx0 = -dG3 */
-  const double gt = -in.u[3] * in.u[3] * gm.dG3;
+  const double gt = H ? 0.0 : -in.u[3] * in.u[3] * gm.dG3;
   du[0] = -(in.ulo[1] * du[1] + in.ulo[2] * du[2] + in.ulo[3] * du[3]) * igam - gt * (0.5 * igam);
 #pragma unroll
   for (int m = 0; m < 4; ++m) dulo[m] = in.glo[m] * du[m];
-  dulo[3] += -gm.dG3 * in.u[3];
+  if (!H) dulo[3] += -gm.dG3 * in.u[3];
   o.du0 = du[0];
-  const double theta = in.thc + du[0];
+  const double theta = H ? du[0] : in.thc + du[0];
   o.theta = theta;
   /* covariant derivative, acceleration */
   double CD[4][4], Du[4], Dulo[4];
 #pragma unroll
   for (int m = 0; m < 4; ++m)
 #pragma unroll
-    for (int n = 0; n < 4; ++n) CD[m][n] = in.CDc[m][n];
+    for (int n = 0; n < 4; ++n) CD[m][n] = H ? 0.0 : in.CDc[m][n];
 #pragma unroll
-  for (int n = 0; n < 4; ++n) { CD[0][n] += du[n]; Du[n] = in.Duc[n] + gam * du[n]; Dulo[n] = in.glo[n] * Du[n]; }
+  for (int n = 0; n < 4; ++n) { CD[0][n] += du[n]; Du[n] = (H ? 0.0 : in.Duc[n]) + gam * du[n]; Dulo[n] = in.glo[n] * Du[n]; }
 
   const double Pi = in.ds.bulkt * sig;
   const bool need_sg = kp.shear || (kp.bulk && in.lambda_Pipi != 0.0) || sgsq_out != nullptr;
@@ -97,7 +103,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
   /* bulk */
   o.dBulk = 0.0;
   if (kp.bulk) {
-    double rhs = -Pi - in.zeta * theta + (in.tau_Pi - in.delta_PiPi) * Pi * theta;
+    double rhs = -K * Pi - in.zeta * theta + (in.tau_Pi - in.delta_PiPi) * Pi * theta;
     if (in.lambda_Pipi != 0.0) {
       double acc = 0.0;
 #pragma unroll
@@ -134,7 +140,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
       for (int j = i; j <= 3; ++j) {
         if (D == 2 && j == 3 && i != 3) continue;          /* pi^{13}, pi^{23} vanish by symmetry in 2+1D */
         double conn = 0.0;                                  /* u^l Gamma^i_{l r} pi~^{r j} + (i <-> j)      */
-        if (gm.hyper) {
+        if (gm.hyper && !H) {
           if (i == 3) conn += (gam * in.ds.pit[3][j] + in.u[3] * in.ds.pit[0][j]) * itau;
           if (j == 3) conn += (gam * in.ds.pit[i][3] + in.u[3] * in.ds.pit[i][0]) * itau;
         }
@@ -142,7 +148,7 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
 #pragma unroll
         for (int l = 0; l < 4; ++l) acc += (in.u[i] * in.ds.pit[j][l] + in.u[j] * in.ds.pit[i][l]) * Dulo[l];
         const double piij = sig * in.ds.pit[i][j];
-        double rhs = -piij + 2.0 * in.eta * sg[i][j] + (in.tau_pi - in.delta_pipi) * piij * theta;
+        double rhs = -K * piij + 2.0 * in.eta * sg[i][j] + (in.tau_pi - in.delta_pipi) * piij * theta;
         if (in.tau_pipi != 0.0) {
           double X = 0.0;
 #pragma unroll
@@ -198,8 +204,8 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
 #pragma unroll
       for (int i = 1; i <= D; ++i) {
         double conn = 0.0;
-        if (gm.hyper && i == 3) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) * itau;
-        o.dJt[q][i] = (in.rhsJ[q][i - 1] * in.i_tauq_sig[q] - conn - in.u[i] * JDu) * igam;
+        if (gm.hyper && i == 3 && !H) conn = (gam * in.ds.Jt[q][3] + in.u[3] * in.ds.Jt[q][0]) * itau;
+        o.dJt[q][i] = (H ? -in.u[i] * JDu : in.rhsJ[q][i - 1] * in.i_tauq_sig[q] - conn - in.u[i] * JDu) * igam;
       }
       double acc = 0.0;
 #pragma unroll
@@ -212,10 +218,10 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
   /* charge: d/dx0 [ N_q + J~^0_q / gamma ] = -sqrt(-g) FK_q */
 #pragma unroll
   for (int q = 0; q < NQ; ++q)
-    o.dN[q] = -in.FKs[q] - o.dJt[q][0] * igam + (in.ds.Jt[q][0] * (igam * igam)) * du[0];
+    o.dN[q] = -K * in.FKs[q] - o.dJt[q][0] * igam + (in.ds.Jt[q][0] * (igam * igam)) * du[0];
   /* entropy, Eq. 96: gamma sigma (T dS + mu_q dN_q) = -Pi theta + pi^mu_nu nabla_mu u^nu */
   {
-    double rhs = -Pi * theta + in.uI;
+    double rhs = -Pi * theta + K * in.uI;
     if (kp.shear)
 #pragma unroll
       for (int m = 0; m < 4; ++m)
@@ -237,8 +243,8 @@ __device__ __forceinline__ void eom_rates(const KParams& kp, const Geom& gm, con
   for (int i = 1; i <= D; ++i) {
     const double pit0_lo = in.glo[i] * in.ds.pit[0][i];
     double dpit0_lo = in.glo[i] * o.dpit[0][i];
-    if (i == 3) dpit0_lo += -gm.dG3 * in.ds.pit[0][3];
-    o.res[i - 1] = in.ulo[i] * dC + Cc * dulo[i] + dpit0_lo * igam - (pit0_lo * (igam * igam)) * du[0] - in.FM[i - 1];
+    if (i == 3 && !H) dpit0_lo += -gm.dG3 * in.ds.pit[0][3];
+    o.res[i - 1] = in.ulo[i] * dC + Cc * dulo[i] + dpit0_lo * igam - (pit0_lo * (igam * igam)) * du[0] - K * in.FM[i - 1];
   }
 }
 
@@ -402,21 +408,20 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
   /* residual at du = 0 and at the unit vectors -> D x D system of Eq. 95 */
   EomOut o;
   double r0[3], M[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}}, du[3] = {0.0, 0.0, 0.0};
-  eom_rates<D>(kp, gm, in, du, o);
+  eom_rates<D, 1>(kp, gm, in, du, o);
 #pragma unroll
   for (int k = 0; k < D; ++k) r0[k] = o.res[k];
-  /* one copy of the rate evaluation for all D columns (the instruction cache matters: the evaluation is a few
-     thousand instructions); unit vector and column store by selects, so no array is indexed dynamically */
-#pragma unroll 1
-  for (int c = 0; c < D; ++c) {
-    const double e[3] = {c == 0 ? 1.0 : 0.0, c == 1 ? 1.0 : 0.0, c == 2 ? 1.0 : 0.0};
-    eom_rates<D>(kp, gm, in, e, o);
+  /* columns of the matrix: the homogeneous part of the map at e_c, each a specialised (much shorter) evaluation */
+  eom_rates<D, 2>(kp, gm, in, du, o);
 #pragma unroll
-    for (int k = 0; k < D; ++k) {
-      const double m = o.res[k] - r0[k];
+  for (int k = 0; k < D; ++k) M[k][0] = o.res[k];
+  eom_rates<D, 3>(kp, gm, in, du, o);
 #pragma unroll
-      for (int cc = 0; cc < D; ++cc) M[k][cc] = (cc == c) ? m : M[k][cc];
-    }
+  for (int k = 0; k < D; ++k) M[k][1] = o.res[k];
+  if (D == 3) {
+    eom_rates<D, 4>(kp, gm, in, du, o);
+#pragma unroll
+    for (int k = 0; k < D; ++k) M[k][2] = o.res[k];
   }
   /* Gaussian elimination with partial pivoting */
   double b[3];
@@ -451,7 +456,7 @@ eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, u
       du[r] = s0 / M[r][r];
     }
   double sgsq = 0.0;
-  eom_rates<D>(kp, gm, in, du, o, DIAG ? &sgsq : nullptr);
+  eom_rates<D, 0>(kp, gm, in, du, o, DIAG ? &sgsq : nullptr);
   if (DIAG) {                                      /* applicability diagnostics, Eq. 58-61 (:797-805) */
     double pp = 0.0;
 #pragma unroll

@@ -172,6 +172,231 @@ eos_invert_kernel(KParams kp, InvertArgs a, int64_t nodes, double* __restrict__ 
     if (a.col_of[c] >= 0) o[a.col_of[c]] = v[c];
 }
 
+/* Rest of NEXT-1: the offline inverter on a TABULATED forward EoS (PAPER.md :576-593; DESIGN reading 21) — what the paper
+   runs on the host because "root-finding for non-linear functions is not tractable on GPUs" (:585).  One thread per
+   node of the (s, B, S, Q) target grid: damped 4-D Newton on the quadrilinear interpolant of the forward table
+   (p, s, n_B, n_S, n_Q)(T, mu_B, mu_S, mu_Q); a node the root-finder does not reach takes the backup EoS (:572), the
+   closed-form conformal family of the context, and is flagged. */
+struct FwdDev {
+  int dims[4];
+  const double* ax[4];
+  const double* data;      /* [node][5] */
+};
+
+/* interpolant and its Jacobian by successive 1-D reductions (axis 3 first): v = lo + t (hi - lo); the slope along the
+   reduced axis is (hi - lo) / width, slopes along axes reduced earlier are blended like the values.
+   Y[0..4] = p, s, n_q; J[i][k] = d Y[1 + i] / d X_k. */
+__device__ inline void fwd_eval(const FwdDev& f, const double X[4], double Y[5], double J[4][4]) {
+  int i0[4];
+  double t[4], iw[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const double* ax = f.ax[k];
+    const int nn = f.dims[k];
+    double xv = X[k];
+    if (!(xv >= ax[0])) xv = ax[0];
+    if (!(xv <= ax[nn - 1])) xv = ax[nn - 1];
+    const int i = axis_cell(ax, nn, xv);
+    i0[k] = i;
+    const double lo = ax[i], w = ax[i + 1] - lo;
+    t[k] = (xv - lo) / w;
+    iw[k] = 1.0 / w;
+  }
+#pragma unroll
+  for (int c = 0; c < 5; ++c) {
+    /* level 3 -> 8 values + slope along axis 3 */
+    double v3[8], d3[8];
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const int64_t node = (((int64_t)(i0[0] + (b >> 2)) * f.dims[1] + (i0[1] + ((b >> 1) & 1))) * f.dims[2] + (i0[2] + (b & 1))) * f.dims[3] + i0[3];
+      const double lo = __ldg(f.data + node * 5 + c), hi = __ldg(f.data + (node + 1) * 5 + c);
+      const double df = hi - lo;
+      v3[b] = fma(t[3], df, lo);
+      d3[b] = df * iw[3];
+    }
+    double v2[4], d32[4], d2[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const double df = v3[2 * b + 1] - v3[2 * b];
+      v2[b] = fma(t[2], df, v3[2 * b]);
+      d2[b] = df * iw[2];
+      d32[b] = fma(t[2], d3[2 * b + 1] - d3[2 * b], d3[2 * b]);
+    }
+    double v1[2], d31[2], d21[2], d1[2];
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const double df = v2[2 * b + 1] - v2[2 * b];
+      v1[b] = fma(t[1], df, v2[2 * b]);
+      d1[b] = df * iw[1];
+      d21[b] = fma(t[1], d2[2 * b + 1] - d2[2 * b], d2[2 * b]);
+      d31[b] = fma(t[1], d32[2 * b + 1] - d32[2 * b], d32[2 * b]);
+    }
+    const double df = v1[1] - v1[0];
+    Y[c] = fma(t[0], df, v1[0]);
+    if (c >= 1) {
+      J[c - 1][0] = df * iw[0];
+      J[c - 1][1] = fma(t[0], d1[1] - d1[0], d1[0]);
+      J[c - 1][2] = fma(t[0], d21[1] - d21[0], d21[0]);
+      J[c - 1][3] = fma(t[0], d31[1] - d31[0], d31[0]);
+    }
+  }
+}
+
+/* x = A^-1 b (transpose = false) or A^-T b, 4 x 4, elimination with partial pivoting; false if singular */
+__device__ inline bool solve4(const double Ain[4][4], const double bin[4], bool transpose, double x[4]) {
+  double A[4][5];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) A[i][k] = transpose ? Ain[k][i] : Ain[i][k];
+    A[i][4] = bin[i];
+  }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    int piv = c;
+#pragma unroll
+    for (int r = c + 1; r < 4; ++r) if (fabs(A[r][c]) > fabs(A[piv][c])) piv = r;
+    if (A[piv][c] == 0.0) return false;
+#pragma unroll
+    for (int r = c + 1; r < 4; ++r)
+      if (r == piv) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) { const double tmp = A[c][k]; A[c][k] = A[r][k]; A[r][k] = tmp; }
+      }
+    const double inv = 1.0 / A[c][c];
+#pragma unroll
+    for (int r = c + 1; r < 4; ++r) {
+      const double fct = A[r][c] * inv;
+#pragma unroll
+      for (int k = c; k < 5; ++k) A[r][k] = fma(-fct, A[c][k], A[r][k]);
+    }
+  }
+#pragma unroll
+  for (int r = 3; r >= 0; --r) {
+    double acc = A[r][4];
+#pragma unroll
+    for (int k = r + 1; k < 4; ++k) acc = fma(-A[r][k], x[k], acc);
+    x[r] = acc / A[r][r];
+  }
+  return true;
+}
+
+__device__ inline ThermoOut eos_invert_forward(const KParams& kp, const FwdDev& f, double s, const double n[NQ], int& flag) {
+  const double Ys[4] = {s, n[0], n[1], n[2]};
+  const double inv_s = 1.0 / s;
+  double X[4], Y[5], J[4][4];
+  auto clampX = [&](double* x) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) x[k] = fmin(fmax(x[k], f.ax[k][0]), f.ax[k][f.dims[k] - 1]);
+  };
+  auto res2 = [&](const double* y) {
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const double d = (y[1 + i] - Ys[i]) * inv_s; r = fma(d, d, r); }
+    return r;
+  };
+  auto rmax = [&](const double* y) {
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) r = fmax(r, fabs(y[1 + i] - Ys[i]));
+    return r;
+  };
+  X[0] = X[1] = X[2] = X[3] = 0.0;
+  clampX(X);
+  {
+    double lo = f.ax[0][0], hi = f.ax[0][f.dims[0] - 1];
+    for (int it = 0; it < 60; ++it) {
+      X[0] = 0.5 * (lo + hi);
+      fwd_eval(f, X, Y, J);
+      if (Y[1] > s) hi = X[0]; else lo = X[0];
+    }
+    X[0] = 0.5 * (lo + hi);
+  }
+  fwd_eval(f, X, Y, J);
+  bool ok = false;
+  const double tol = 1e-13 * s;
+  for (int it = 0; it < 40; ++it) {
+    if (rmax(Y) <= tol) { ok = true; break; }
+    double rhs[4], d[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) rhs[i] = -(Y[1 + i] - Ys[i]);
+    if (!solve4(J, rhs, false, d)) break;
+    const double r0 = res2(Y);
+    double lam = 1.0;
+    bool acc = false;
+    for (int hv = 0; hv <= 12; ++hv) {
+      double Xn[4], Yn[5], Jn[4][4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Xn[k] = X[k] + lam * d[k];       /* no contraction: as the oracle steps */
+      clampX(Xn);
+      fwd_eval(f, Xn, Yn, Jn);
+      if (res2(Yn) < r0) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) X[k] = Xn[k];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) Y[c] = Yn[c];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int k = 0; k < 4; ++k) J[i][k] = Jn[i][k];
+        acc = true;
+        break;
+      }
+      lam *= 0.5;
+    }
+    if (!acc) break;
+  }
+  if (!ok) ok = rmax(Y) <= tol;
+  double z[4], v[4];
+  if (ok) ok = solve4(J, Ys, true, z);
+  if (ok) ok = solve4(J, Ys, false, v);
+  if (!ok) {
+    flag = 1;
+    return eos_closed_form(kp, s, n);
+  }
+  flag = 0;
+  ThermoOut th;
+  th.oob = 0;
+  th.T = X[0];
+  for (int q = 0; q < NQ; ++q) { th.mu[q] = X[1 + q]; th.wq[q] = X[1 + q] + z[1 + q]; }
+  th.p = Y[0];
+  th.e = X[0] * s - Y[0] + (X[1] * n[0] + X[2] * n[1] + X[3] * n[2]);
+  th.ws = X[0] + z[0];
+  double num = 0.0, den = 0.0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { num += Ys[i] * v[i]; den += X[i] * Ys[i]; }
+  th.cs2 = num / den;
+  return th;
+}
+
+__global__ void __launch_bounds__(128)
+eos_invert_fwd_kernel(KParams kp, InvertArgs a, FwdDev f, int64_t nodes, double* __restrict__ data, int* __restrict__ flags,
+                      unsigned long long* __restrict__ n_backup) {
+  const int64_t node = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (node >= nodes) return;
+  int64_t r = node;
+  const int i3 = (int)(r % a.dims[3]); r /= a.dims[3];
+  const int i2 = (int)(r % a.dims[2]); r /= a.dims[2];
+  const int i1 = (int)(r % a.dims[1]); r /= a.dims[1];
+  const int i0 = (int)r;
+  const double s = a.ax[0][i0];
+  const double y[NQ] = {a.ax[1][i1], a.ax[2][i2], a.ax[3][i3]};
+  double n[NQ];
+  for (int q = 0; q < NQ; ++q) n[q] = (a.kind[q + 1] == 1) ? y[q] * s : y[q];
+  int flag = 0;
+  const ThermoOut th = eos_invert_forward(kp, f, s, n, flag);
+  if (flags) flags[node] = flag;
+  if (flag) atomicAdd(n_backup, 1ULL);
+  double v[CCAKE_NCOLS_MAX];
+  v[CCAKE_COL_T] = th.T;
+  for (int q = 0; q < NQ; ++q) { v[CCAKE_COL_MUB + q] = th.mu[q]; v[CCAKE_COL_WB + q] = th.wq[q]; }
+  v[CCAKE_COL_P] = th.p; v[CCAKE_COL_CS2] = th.cs2; v[CCAKE_COL_E] = th.e; v[CCAKE_COL_WS] = th.ws;
+  double* __restrict__ o = data + node * a.ncols;
+#pragma unroll
+  for (int c = 0; c < CCAKE_NCOLS_MAX; ++c)
+    if (a.col_of[c] >= 0) o[a.col_of[c]] = v[c];
+}
+
 /* dissipative tensors of one particle: evolved spatial components from the store, time components from
    u_mu pi^{mu nu} = 0 and u_mu J^mu = 0 (never evolved; DESIGN reading 13) */
 struct Dissip { double pit[4][4], Jt[NQ][4], bulkt; };

@@ -163,6 +163,26 @@ def make_eos_table(ns=100, nq=32, ymax=0.05, with_wq=False, c0=EOS_C0, c2=EOS_C2
     return dict(axes=[s_ax, y_ax, y_ax, y_ax], axis_kind=[0, 1, 1, 1], col_ids=list(range(ncols)), data=data)
 
 
+def signed_geometric_axis(n: int, xmax: float, xmin: float):
+    """n nodes: -xmax ... -xmin (geometric, n // 2 - 1 ... nodes), 0, +xmin ... +xmax (geometric): log-scaled on both sides
+    of zero, as (T, mu) tables that have to serve many decades of temperature are."""
+    nneg = (n - 1) // 2
+    npos = n - 1 - nneg
+    return np.concatenate([-np.geomspace(xmax, xmin, nneg), [0.0], np.geomspace(xmin, xmax, npos)])
+
+
+def make_forward_table(nT=100, nmu=32, T_lo=5e-4, T_hi=4.0, mu_lo=1e-5, mu_hi=4.4, c0=EOS_C0, c2=EOS_C2, c4=EOS_C4):
+    """Input of the offline inverter (BASELINE.json configs[1]: "tabulated forward on a 100x32x32x32 (T, mu_B, mu_S, mu_Q)
+    grid"): (p, s, n_B, n_S, n_Q) of the analytic conformal BSQ pressure at the nodes of a geometric T axis and three
+    signed-geometric mu axes.  Returns dict(axes=[T, mu, mu, mu], data[nT, nmu, nmu, nmu, 5])."""
+    T_ax = np.geomspace(T_lo, T_hi, nT)
+    m_ax = signed_geometric_axis(nmu, mu_hi, mu_lo)
+    T, mB, mS, mQ = np.meshgrid(T_ax, m_ax, m_ax, m_ax, indexing="ij")
+    p, s, n = conformal_forward(T, np.stack([mB, mS, mQ]), c0, c2, c4)
+    data = np.stack([p, s, n[0], n[1], n[2]], axis=-1)
+    return dict(axes=[T_ax, m_ax, m_ax, m_ax], data=np.ascontiguousarray(data))
+
+
 # ------------------------------------------------------------------------------------------- Gubser configs ---
 def _square_lattice(n, dx):
     x1 = (np.arange(n) - 0.5 * (n - 1)) * dx
