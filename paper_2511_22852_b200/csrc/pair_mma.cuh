@@ -520,20 +520,33 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   if (tid < NW) done_turn[tid] = -1;
   __syncthreads();
 
-  /* byte offsets of this lane's B operands inside a staged record: column gid of tile T for weight j */
+  /* byte offsets of this lane's B operands inside a staged record: column gid of tile T for weight j.  They live in
+     a small table in shared memory and are read back in front of every quad loop: kept in registers across the
+     culling and compaction code the compiler recomputed them per tile with a chain of ~60 selects */
   const uint32_t pay_s = (uint32_t)__cvta_generic_to_shared(pay);
   const uint32_t payx_s = (uint32_t)__cvta_generic_to_shared(payx);
+  __shared__ uint32_t s_boff[NT * NJ][8];
+  if (tid < 8) {
+#pragma unroll
+    for (int T = 0; T < NT; ++T)
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        int e = ELEM_NONE;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) if (c == tid) e = Op::elem(T, j, c);
+        if (e < 0) e = 0;                            /* unused column: any finite element; its sums are dropped */
+        s_boff[T * NJ + j][tid] = (uint32_t)((e >> 1) * CSTRIDE) * 16u + (uint32_t)(e & 1) * 8u;
+      }
+  }
+  __syncthreads();
   uint32_t boff[NT][NJ];
+  auto load_boff = [&]() {
 #pragma unroll
-  for (int T = 0; T < NT; ++T)
+    for (int T = 0; T < NT; ++T)
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-      int e = ELEM_NONE;
-#pragma unroll
-      for (int c = 0; c < 8; ++c) if (c == gid) e = Op::elem(T, j, c);
-      if (e < 0) e = 0;                              /* unused column: any finite element; its sums are dropped */
-      boff[T][j] = (uint32_t)((e >> 1) * CSTRIDE) * 16u + (uint32_t)(e & 1) * 8u;
-    }
+      for (int j = 0; j < NJ; ++j) boff[T][j] = *reinterpret_cast<volatile uint32_t*>(&s_boff[T * NJ + j][gid]);
+  };
+  load_boff();
 
   double acc[GPW][NT][NJ][2];
 #pragma unroll
@@ -701,6 +714,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
         }
         __syncwarp();
         /* full quads, then one partial quad (idle lanes re-read its first candidate with weight 0) */
+        load_boff();
         uint32_t nibs = 0u;                                       /* lane q: the 4 union bits of quad q */
         const int nfull = tl >> 2;
         const uint16_t* fq = ff + tig;
