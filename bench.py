@@ -383,6 +383,7 @@ def run_ours(args):
                    "cpu_oracle_nodes_per_s": nsample / t_cpu, "cpu_sample": f"{nsample} seeded nodes, 1 thread, through ctypes"}
         # rest of NEXT-1: the same target grid from a TABULATED forward EoS (BASELINE.json configs[1]: 100 x 32^3 (T, mu) grid),
         # damped 4-D Newton per node on the device; the oracle's inverter on a seeded sample of nodes beside it
+        from paper_2511_22852_b200 import workloads as W
         ft = W.make_forward_table(100, 32)
         sim.invert_forward_table(ft["axes"], ft["data"], tb["axes"], tb["axis_kind"], tb["col_ids"])      # warm-up
         t0 = time.perf_counter()

@@ -59,7 +59,8 @@ struct ccake_ctx {
   int cand_cap = 0;
   uint32_t* nnb = nullptr;
   double* theta = nullptr;
-  double* scratch = nullptr;    /* N doubles: read_fields staging */
+  double* scratch = nullptr;    /* N doubles: staging of ccake_read_neighbors */
+  double* stage = nullptr;      /* STAGE_FIELDS x npad doubles: staging of ccake_read_fields into host buffers (on first use) */
   double* src = nullptr;        /* 7 x npad, original order: I^mu, I_q of ccake_set_sources (allocated on first use) */
   bool has_src = false;
   Sorted so;
@@ -74,6 +75,14 @@ struct ccake_ctx {
   int64_t substeps_timed = 0;
 
   int64_t launches = 0;   /* kernels enqueued since the last ccake_launch_count() */
+
+  /* the current time on the device (read by the thermo and EoM kernels, advanced by the last kernel of a step), so that
+     a full RK step is a fixed launch sequence with fixed arguments and can be captured once as a CUDA graph and
+     replayed.  One graph per physical buffer that holds Y[0]: the reorder of the first substep swaps Y[0] and Y[1]. */
+  double* x0_dev = nullptr;
+  struct StepGraph { const double* y0; cudaGraphExec_t exec; int64_t launches; };
+  std::vector<StepGraph> graphs;
+  bool use_graphs = true;
 
   std::string err;
 };
@@ -91,7 +100,10 @@ namespace {
 
 inline int nblk(int64_t n, int t) { return (int)((n + t - 1) / t); }
 
+void drop_graphs(ccake_ctx* c);
+
 void free_particles(ccake_ctx* c) {
+  drop_graphs(c);
   for (int k = 0; k < 3; ++k) { cudaFree(c->Y[k]); c->Y[k] = nullptr; }
   cudaFree(c->Krate); c->Krate = nullptr;
   for (int k = 0; k < 2; ++k) {
@@ -113,6 +125,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->nnb); c->nnb = nullptr;
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
+  cudaFree(c->stage); c->stage = nullptr;
   cudaFree(c->src); c->src = nullptr; c->has_src = false;
   c->loaded = false;
 }
@@ -214,12 +227,19 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
   return launch_check(c, "build_cells");
 }
 
+__global__ void set_time_kernel(double* x0_dev, double x0) { *x0_dev = x0; }
+__global__ void advance_time_kernel(double* x0_dev, double dt) { *x0_dev = *x0_dev + dt; }
+
+void drop_graphs(ccake_ctx* c) {
+  for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+  c->graphs.clear();
+}
+
 template <int D>
-int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
+int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in) {
   const int64_t N = c->N, np = c->npad;
   cudaStream_t st = c->stream;
   const KParams& kp = c->kp;
-  const Geom gm = make_geom(c->P.coords, x0s);
   int rc;
   pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->grid, c->so);
   if ((rc = mark(c))) return rc;
@@ -232,7 +252,7 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   if ((rc = mark(c))) return rc;
   /* a5 */
   cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
-  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, c->tb, Ycur, np, c->so, c->status, rk_in.update);
+  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, c->tb, Ycur, np, c->so, c->status, rk_in.update);
   if ((rc = mark(c))) return rc;
   /* a6 */
   launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
@@ -243,20 +263,20 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk_in) {
   rk.theta_out = c->theta;
   rk.src = c->has_src ? c->src : nullptr;
   rk.orig = c->orig[0];
-  if (rk.diag) eom_kernel<D, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
-  else eom_kernel<D, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, gm, np, c->so, rk, c->field_mask, c->status);
+  if (rk.diag) eom_kernel<D, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, np, c->so, rk, c->field_mask, c->status);
+  else eom_kernel<D, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, np, c->so, rk, c->field_mask, c->status);
   if ((rc = mark(c))) return rc;
   c->launches += 5;
   return launch_check(c, "substep");
 }
 
-int substep(ccake_ctx* c, double* Ycur, double x0s, const RkArgs& rk) {
+int substep(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk) {
   int rc;
   if ((rc = mark(c))) return rc;
   if ((rc = build_cells(c, Ycur, false))) return rc;
   if ((rc = mark(c))) return rc;
-  if (c->P.dim == 2) rc = pair_and_eom<2>(c, Ycur, x0s, rk);
-  else rc = pair_and_eom<3>(c, Ycur, x0s, rk);
+  if (c->P.dim == 2) rc = pair_and_eom<2>(c, Ycur, x0_off, rk);
+  else rc = pair_and_eom<3>(c, Ycur, x0_off, rk);
   if (c->timing) c->substeps_timed++;
   return rc;
 }
@@ -279,12 +299,12 @@ int rk_step(ccake_ctx* c) {
       if ((rc = build_cells(c, Ycur, true))) return rc;
       if ((rc = mark(c))) return rc;
       rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
-      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, x0, rk) : pair_and_eom<3>(c, Ycur, x0, rk);
+      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
       if (rc) return rc;
       if (c->timing) c->substeps_timed++;
     }
     rk.c_out = dt; rk.Ybase = c->Y[0]; rk.Yout = c->Y[0];
-    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
   } else {
     rk.Yacc = c->Y[2];
     {
@@ -293,18 +313,20 @@ int rk_step(ccake_ctx* c) {
       if ((rc = build_cells(c, Ycur, true))) return rc;
       if ((rc = mark(c))) return rc;
       rk.Ybase = c->Y[0]; rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt; rk.acc_mode = 1; rk.w_acc = 1.0;
-      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, x0, rk) : pair_and_eom<3>(c, Ycur, x0, rk);
+      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
       if (rc) return rc;
       if (c->timing) c->substeps_timed++;
     }
     rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
     rk.c_out = 0.5 * dt; rk.acc_mode = 2; rk.w_acc = 2.0;
-    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
     rk.c_out = dt;
-    if ((rc = substep(c, c->Y[1], x0 + 0.5 * dt, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
     rk.Yout = c->Y[0]; rk.c_out = dt / 6.0; rk.acc_mode = 3;
-    if ((rc = substep(c, c->Y[1], x0 + dt, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], dt, rk))) return rc;
   }
+  advance_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, dt);      /* x0 <- x0 + dt, the same operation as on the host below */
+  c->launches += 1;
   c->x0 = x0 + dt;
   c->derived_valid = false;
   return CCAKE_OK;
@@ -437,7 +459,7 @@ int refresh(ccake_ctx* c) {
   int rc = build_cells(c, Ycur, true);
   if (!rc) {
     rk.Ybase = c->Y[0]; rk.Yout = c->Y[0];
-    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, c->x0, rk) : pair_and_eom<3>(c, Ycur, c->x0, rk);
+    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
   }
   c->timing = t;
   if (rc) return rc;
@@ -610,12 +632,16 @@ int ccake_create(const ccake_params* p, ccake_ctx** out) {
     for (int q = 0; q < 3; ++q) for (int j = 0; j < p->dim; ++j) on(CCAKE_JB1 + 3 * q + j);
   if (p->coords == 1 && p->dim == 2) on(CCAKE_WORK);
   c->field_mask = m;
-  if (cudaMalloc(&c->grid, sizeof(Grid)) != cudaSuccess || cudaMalloc(&c->status, sizeof(Status)) != cudaSuccess) {
+  if (cudaMalloc(&c->grid, sizeof(Grid)) != cudaSuccess || cudaMalloc(&c->status, sizeof(Status)) != cudaSuccess ||
+      cudaMalloc(&c->x0_dev, sizeof(double)) != cudaSuccess) {
     cudaFree(c->grid);
+    cudaFree(c->status);
     delete c;
     return CCAKE_ENOMEM;
   }
   cudaMemset(c->status, 0, sizeof(Status));
+  cudaMemcpy(c->x0_dev, &c->x0, sizeof(double), cudaMemcpyHostToDevice);
+  c->use_graphs = (c->stream != nullptr) && std::getenv("CCAKE_NO_GRAPH") == nullptr;   /* the legacy default stream cannot be captured */
   *out = c;
   return CCAKE_OK;
 }
@@ -628,6 +654,7 @@ int ccake_destroy(ccake_ctx* c) {
   free_table(c);
   cudaFree(c->grid);
   cudaFree(c->status);
+  cudaFree(c->x0_dev);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   delete c;
   return CCAKE_OK;
@@ -648,6 +675,8 @@ static int reload_particles(ccake_ctx* c, int32_t nfields, const int32_t* ids, c
   CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
   c->launches += 2;
   c->x0 = c->P.x0_start;
+  set_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, c->x0);
+  if (c->has_src) drop_graphs(c);       /* the captured steps read the sources of the previous load */
   c->derived_valid = false;
   c->has_src = false;
   return launch_check(c, "reload");
@@ -745,6 +774,7 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   CK(cudaMalloc(&c->cell_start, sizeof(uint32_t) * ((size_t)c->max_cells + 2)));
   carve(c);
   c->x0 = c->P.x0_start;
+  set_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, c->x0);
   c->loaded = true;
   c->derived_valid = false;
   int rc = launch_check(c, "load");
@@ -790,6 +820,7 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
       off += dims[k];
     }
   }
+  drop_graphs(c);
   free_table(c);
   CK(cudaMalloc(&c->tb_axes, sizeof(double) * nax));
   CK(cudaMalloc(&c->tb_data, sizeof(double) * nodes * ncols));
@@ -804,6 +835,7 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
   tb.ncols = ncols;
   tb.data = c->tb_data;
   c->tb = tb;
+  drop_graphs(c);
   c->table_loaded = true;
   c->derived_valid = false;
   return CCAKE_OK;
@@ -1000,6 +1032,7 @@ int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* cons
   bool any = false;
   for (int m = 0; m < 7; ++m) any = any || ((m < 4) ? (I && I[m]) : (Iq && Iq[m - 4]));
   c->derived_valid = false;
+  if (any != c->has_src) drop_graphs(c);            /* the captured steps were recorded with / without the source columns */
   if (!any) { c->has_src = false; return CCAKE_OK; }
   const int64_t np = c->npad, n = c->N;
   if (!c->src) CK(cudaMalloc(&c->src, sizeof(double) * 7 * np));
@@ -1020,8 +1053,42 @@ int ccake_step(ccake_ctx* c, int32_t nsteps) {
   if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "step before load"; return CCAKE_ESTATE; }
   CK(cudaSetDevice(c->device));
   for (int s = 0; s < nsteps; ++s) {
-    int rc = rk_step(c);
-    if (rc) return rc;
+    if (!c->use_graphs || c->timing) {              /* per-kernel timing needs the events between the launches */
+      int rc = rk_step(c);
+      if (rc) return rc;
+      continue;
+    }
+    /* one RK step = a fixed launch sequence with fixed arguments (the time is read from device memory): captured once per
+       physical buffer holding Y[0] and replayed; the host-side bookkeeping of rk_step is repeated by hand on a replay */
+    const double* y0 = c->Y[0];
+    ccake_ctx::StepGraph* g = nullptr;
+    for (auto& e : c->graphs) if (e.y0 == y0) g = &e;
+    if (!g) {
+      const int64_t l0 = c->launches;
+      CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+      const int rc = rk_step(c);
+      cudaGraph_t graph = nullptr;
+      const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+      if (rc || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        if (!rc) { c->err = std::string("step capture: ") + cudaGetErrorString(e); return CCAKE_ECUDA; }
+        return rc;
+      }
+      cudaGraphExec_t exec = nullptr;
+      const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+      cudaGraphDestroy(graph);
+      if (ei != cudaSuccess) { c->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ei); return CCAKE_ECUDA; }
+      c->graphs.push_back({y0, exec, c->launches - l0});
+      CK(cudaGraphLaunch(exec, c->stream));
+    } else {
+      CK(cudaGraphLaunch(g->exec, c->stream));
+      std::swap(c->Y[0], c->Y[1]);                  /* as build_cells(reorder) and rk_step do */
+      std::swap(c->orig[0], c->orig[1]);
+      c->launches += g->launches;
+      c->x0 = c->x0 + c->P.dx0;
+      c->derived_valid = false;
+    }
   }
   return CCAKE_OK;
 }
@@ -1060,9 +1127,13 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
   cudaStream_t st = c->stream;
   const Sorted& so = c->so;
   const Geom gm = make_geom(c->P.coords, c->x0);
+  /* host buffers: the fields are gathered into a staging arena STAGE_FIELDS at a time, copied out with one
+     cudaMemcpyAsync each and ONE synchronisation per batch */
+  constexpr int STAGE_FIELDS = 8;
+  if (memspace == CCAKE_HOST && !c->stage) CK(cudaMalloc(&c->stage, sizeof(double) * np * STAGE_FIELDS));
   for (int k = 0; k < nfields; ++k) {
     const int id = ids[k];
-    double* dst = (memspace == CCAKE_DEVICE) ? cols[k] : c->scratch;
+    double* dst = (memspace == CCAKE_DEVICE) ? cols[k] : c->stage + (int64_t)(k % STAGE_FIELDS) * np;
     const int g = nblk(N, 256);
     const double* src_sorted = nullptr;
     if (id >= 0 && id < NSTATE) scatter_store_kernel<<<g, 256, 0, st>>>(c->Y[0] + (int64_t)id * np, c->orig[0], N, dst);
@@ -1099,15 +1170,9 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
       case CCAKE_DIVV: src_sorted = so.divv; break;
       case CCAKE_NNB: scatter_sorted_u32_kernel<<<g, 256, 0, st>>>(so.nnb, so.perm, c->orig[0], N, dst); break;
       case CCAKE_CELL:
-        /* so.FP[2]... are live; use theta-sized temp: reuse Kpair[8] only when diffusion is off — keep it simple: a
-           dedicated pass into so.divv would clobber; allocate nothing, write through scratch2 = so.x-independent */
-        {
-          double* tmp = nullptr;
-          CK(cudaMallocAsync(&tmp, sizeof(double) * np, st));
-          reported_cell_kernel<<<g, 256, 0, st>>>(so.x[0], so.x[1], so.x[2], N, c->P.dim, c->grid, tmp);
-          scatter_sorted_kernel<<<g, 256, 0, st>>>(tmp, so.perm, c->orig[0], N, dst);
-          CK(cudaFreeAsync(tmp, st));
-        }
+        /* the reported cell id is not kept per substep: evaluate it into the read_neighbors scratch column, then scatter */
+        reported_cell_kernel<<<g, 256, 0, st>>>(so.x[0], so.x[1], so.x[2], N, c->P.dim, c->grid, c->scratch);
+        scatter_sorted_kernel<<<g, 256, 0, st>>>(c->scratch, so.perm, c->orig[0], N, dst);
         break;
       case CCAKE_FM1: case CCAKE_FM2: case CCAKE_FM3: {
         const int i = id - CCAKE_FM1;
@@ -1124,8 +1189,8 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
     int rc = launch_check(c, "read_fields");
     if (rc) return rc;
     if (memspace == CCAKE_HOST) {
-      CK(cudaMemcpyAsync(cols[k], c->scratch, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
-      CK(cudaStreamSynchronize(st));
+      CK(cudaMemcpyAsync(cols[k], dst, sizeof(double) * N, cudaMemcpyDeviceToHost, st));
+      if (k % STAGE_FIELDS == STAGE_FIELDS - 1) CK(cudaStreamSynchronize(st));     /* the arena is reused by the next batch */
     }
   }
   CK(cudaStreamSynchronize(st));

@@ -271,10 +271,11 @@ struct RkArgs {
 #endif
 template <int D, bool DIAG>
 __global__ void __launch_bounds__(128, CCAKE_EOM_MINB)
-eom_kernel(int64_t n, KParams kp, Geom gm, int64_t npad, Sorted so, RkArgs rk, uint32_t field_mask,
-           Status* __restrict__ status) {
+eom_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_off, int64_t npad, Sorted so, RkArgs rk,
+           uint32_t field_mask, Status* __restrict__ status) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
+  const Geom gm = make_geom(kp.coords, *x0_dev + x0_off);      /* as the thermo kernel: time of this substep from device memory */
   const int64_t a = so.perm[i];
   const double* Y = rk.Ycur;          /* may alias rk.Yout (RK4 stages 2, 3: own slot read, then written): no __restrict__ */
   EomIn in;

@@ -454,10 +454,11 @@ __device__ inline void load_u(const KParams& kp, const Geom& gm, const double* Y
 }
 
 __global__ void __launch_bounds__(128)
-thermo_kernel(int64_t n, KParams kp, Geom gm, TableDev tb, const double* __restrict__ Y, int64_t npad, Sorted so,
-              Status* __restrict__ status, int on_step) {
+thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_off, TableDev tb, const double* __restrict__ Y,
+              int64_t npad, Sorted so, Status* __restrict__ status, int on_step) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
+  const Geom gm = make_geom(kp.coords, *x0_dev + x0_off);      /* the time lives on the device: a captured step replays */
   const int D = kp.D;
   const int64_t a = so.perm[i];
   double u[4];
