@@ -168,6 +168,43 @@ int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4]
  * ESTATE before a load. */
 int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* const Iq[3], int32_t memspace);
 
+/* ---- Slab decomposition of ONE event over several contexts (not in the paper, which runs one
+ * event per device).  A slab context owns the particles with lo <= r[axis] < hi (lo = -1e300 / hi = +1e300: no neighbour on
+ * that side) and carries ghost copies of the neighbours' particles within halo_width of its faces.  halo_width must cover
+ * two kernel supports plus the drift of a step (>= 4h + 2 dx0): then ONE exchange of particle states per substep suffices —
+ * the context recomputes smoothing sums and thermodynamics of its ghosts, so the gradient sums of every owned particle see
+ * complete neighbours.  The caller moves the messages between contexts (device copy, or NCCL send/recv between ranks):
+ *   per step:  for both sides: export_halo(k=0) -> [transport] -> neighbour.import_ghosts(k=0)     (low side first)
+ *              substep(0);  for k = 1 .. nsub-1:  export_halo(k) -> import_ghosts(k);  substep(k)
+ *              for both sides: export_migrants -> [transport] -> neighbour.import_migrants;  commit
+ * Messages are DEVICE buffers of the caller: 29 rows of buf_cap doubles, row f < 28 = state field f, row 28 = the global
+ * particle id; entry i of every row is particle i of the message, in the sender's store order (deterministic).  Load
+ * indices of a slab context: owned particles 0 .. n_own-1 (after a commit: the stayers in sorted order, then the
+ * arrivals), ghosts behind them; ccake_read_fields returns all of them in that order, ccake_slab_gids their global ids,
+ * ccake_conserved_totals sums over the owned particles only (the caller adds the slabs).  The reported CELL id is relative
+ * to the slab's own bounding box.  A slab context cannot take ccake_step; ESTATE for slab calls on other contexts. */
+int ccake_slab_load(ccake_ctx* c, int64_t n_own, int64_t capacity, int32_t nfields, const int32_t* field_ids,
+                    const double* const* cols, const uint32_t* gids, int32_t axis, double lo, double hi, double halo_width,
+                    int32_t memspace);
+/* side: 0 = the face at lo, 1 = the face at hi.  k = substep about to be evaluated: k = 0 selects the owned particles
+ * within halo_width of the face from the state at the start of the step; k > 0 packs the same particles again from the
+ * stage state.  *count = particles in the message (ENOMEM if it exceeds buf_cap; synchronises the stream). */
+int ccake_slab_export_halo(ccake_ctx* c, int32_t side, int32_t k, double* buf, int64_t buf_cap, int64_t* count);
+/* k = 0: the message becomes the ghosts of this step on that side (the ghosts of the previous step went with the commit);
+ * k > 0: the stage state of those ghosts is overwritten (same count, same order). */
+int ccake_slab_import_ghosts(ccake_ctx* c, int32_t side, int32_t k, const double* buf, int64_t buf_cap, int64_t count);
+/* Substep k (0 .. 1 for RK2, 0 .. 3 for RK4) of one RK step over owned particles and ghosts; the last one advances the time. */
+int ccake_slab_substep(ccake_ctx* c, int32_t k);
+/* After the last substep: the owned particles that left [lo, hi) through `side`, as a message. */
+int ccake_slab_export_migrants(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count);
+int ccake_slab_import_migrants(ccake_ctx* c, int32_t side, const double* buf, int64_t buf_cap, int64_t count);
+/* Rebuild the owned set: stayers (store order) + arrivals from the low side + arrivals from the high side; ghosts dropped. */
+int ccake_slab_commit(ccake_ctx* c, int64_t* n_own_new);
+/* out = { n_own, ghosts from the low side, ghosts from the high side, capacity } */
+int ccake_slab_info(ccake_ctx* c, int64_t out[4]);
+/* Global ids by load index, n_own + ghosts entries. */
+int ccake_slab_gids(ccake_ctx* c, uint32_t* out, int64_t capacity, int32_t memspace);
+
 /* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
 int ccake_step(ccake_ctx* c, int32_t nsteps);
 

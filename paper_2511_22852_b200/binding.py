@@ -32,6 +32,8 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_invert_forward_table", "ccake_smear_sources",
            "ccake_set_sources",
+           "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep",
+           "ccake_slab_export_migrants", "ccake_slab_import_migrants", "ccake_slab_commit", "ccake_slab_info", "ccake_slab_gids",
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
@@ -79,6 +81,15 @@ def lib():
                                                  C.POINTER(i32), vp, vp, C.POINTER(i64), i32]
         L.ccake_smear_sources.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp), i32]
         L.ccake_set_sources.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), i32]
+        L.ccake_slab_load.argtypes = [vp, i64, i64, i32, C.POINTER(i32), C.POINTER(vp), vp, i32, C.c_double, C.c_double, C.c_double, i32]
+        L.ccake_slab_export_halo.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64)]
+        L.ccake_slab_import_ghosts.argtypes = [vp, i32, i32, vp, i64, i64]
+        L.ccake_slab_substep.argtypes = [vp, i32]
+        L.ccake_slab_export_migrants.argtypes = [vp, i32, vp, i64, C.POINTER(i64)]
+        L.ccake_slab_import_migrants.argtypes = [vp, i32, vp, i64, i64]
+        L.ccake_slab_commit.argtypes = [vp, C.POINTER(i64)]
+        L.ccake_slab_info.argtypes = [vp, C.POINTER(i64)]
+        L.ccake_slab_gids.argtypes = [vp, vp, i64, i32]
         L.ccake_step.argtypes = [vp, i32]
         L.ccake_synchronize.argtypes = [vp]
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
@@ -297,6 +308,61 @@ class Ccake:
     def neighbor_hash(self):
         out = np.empty(self.n, dtype=np.uint64)
         self._chk(lib().ccake_neighbor_hash(self._h, out.ctypes.data, self.n), "ccake_neighbor_hash")
+        return out
+
+    # ---- slab decomposition of one event (include/ccake.h, "Slab decomposition"): one call each; messages are torch
+    #      device tensors of shape [29, cap] owned by the caller
+    def slab_load(self, fields: dict, gids, capacity, axis, lo, hi, halo_width):
+        ids = list(fields.keys())
+        trip = [_ptr(fields[k]) for k in ids]
+        assert {t[1] for t in trip} == {HOST}, "slab_load takes host columns"
+        n = int(trip[0][2].shape[0])
+        idarr = (C.c_int32 * len(ids))(*ids)
+        ptrs = (C.c_void_p * len(ids))(*[t[0] for t in trip])
+        g = np.ascontiguousarray(gids, dtype=np.uint32)
+        assert g.size == n
+        self._chk(lib().ccake_slab_load(self._h, n, int(capacity), len(ids), idarr, ptrs, g.ctypes.data, int(axis), float(lo), float(hi),
+                                        float(halo_width), HOST), "ccake_slab_load")
+        self.n = n
+
+    def slab_export_halo(self, side, k, buf):
+        cnt = C.c_int64(0)
+        self._chk(lib().ccake_slab_export_halo(self._h, int(side), int(k), buf.data_ptr(), int(buf.shape[1]), C.byref(cnt)),
+                  "ccake_slab_export_halo")
+        return int(cnt.value)
+
+    def slab_import_ghosts(self, side, k, buf, count):
+        self._chk(lib().ccake_slab_import_ghosts(self._h, int(side), int(k), buf.data_ptr() if buf is not None else None,
+                                                 int(buf.shape[1]) if buf is not None else 0, int(count)), "ccake_slab_import_ghosts")
+        self.n = self.slab_info()[0] + self.slab_info()[1] + self.slab_info()[2]
+
+    def slab_substep(self, k):
+        self._chk(lib().ccake_slab_substep(self._h, int(k)), "ccake_slab_substep")
+
+    def slab_export_migrants(self, side, buf):
+        cnt = C.c_int64(0)
+        self._chk(lib().ccake_slab_export_migrants(self._h, int(side), buf.data_ptr(), int(buf.shape[1]), C.byref(cnt)),
+                  "ccake_slab_export_migrants")
+        return int(cnt.value)
+
+    def slab_import_migrants(self, side, buf, count):
+        self._chk(lib().ccake_slab_import_migrants(self._h, int(side), buf.data_ptr() if buf is not None else None,
+                                                   int(buf.shape[1]) if buf is not None else 0, int(count)), "ccake_slab_import_migrants")
+
+    def slab_commit(self):
+        n = C.c_int64(0)
+        self._chk(lib().ccake_slab_commit(self._h, C.byref(n)), "ccake_slab_commit")
+        self.n = int(n.value)
+        return self.n
+
+    def slab_info(self):
+        out = (C.c_int64 * 4)()
+        self._chk(lib().ccake_slab_info(self._h, out), "ccake_slab_info")
+        return tuple(int(v) for v in out)
+
+    def slab_gids(self):
+        out = np.empty(self.n, dtype=np.uint32)
+        self._chk(lib().ccake_slab_gids(self._h, out.ctypes.data, out.size, HOST), "ccake_slab_gids")
         return out
 
     def enable_timing(self, on=True):

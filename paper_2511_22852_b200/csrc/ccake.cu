@@ -16,6 +16,7 @@
 #include "eom.cuh"
 #include "grid_sort.cuh"
 #include "pair_mma.cuh"
+#include "slab.cuh"
 #include "thermo_eos.cuh"
 #include "totals.cuh"
 
@@ -84,6 +85,22 @@ struct ccake_ctx {
   std::vector<StepGraph> graphs;
   bool use_graphs = true;
 
+  /* slab mode (slab.cuh, ccake_slab_*): this context owns the particles of one slab [slab_lo, slab_hi) along slab_axis of a
+     decomposed event and carries, behind them, ghost copies of the neighbours' particles within slab_w of its faces */
+  bool slab = false;
+  int slab_axis = 0;
+  double slab_lo = 0.0, slab_hi = 0.0, slab_w = 0.0;
+  int64_t n_own = 0, cap = 0;
+  int64_t n_ghost[2] = {0, 0};      /* ghosts imported from the low / high neighbour in this step (low ones first) */
+  int64_t halo_cnt[2] = {0, 0};     /* particles exported to the low / high neighbour in this step */
+  bool inv_valid = false;           /* slot_of[] matches the current store order */
+  uint32_t *gid = nullptr, *gid_new = nullptr;   /* global particle id by load index */
+  uint32_t *slot_of = nullptr;      /* store slot of a load index (inverse of orig) */
+  uint32_t *sflag[3] = {nullptr, nullptr, nullptr}, *stot[3] = {nullptr, nullptr, nullptr};   /* selection flags / ranks, chunk totals */
+  uint32_t *halo_list[2] = {nullptr, nullptr};   /* load indices exported to each side in this step */
+  int64_t mig_in[2] = {0, 0};       /* migrants received from each side, parked behind the ghosts until the commit */
+  double* mig_buf = nullptr;        /* [SLAB_NF][cap]: parked migrants */
+
   std::string err;
 };
 
@@ -127,6 +144,11 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->scratch); c->scratch = nullptr;
   cudaFree(c->stage); c->stage = nullptr;
   cudaFree(c->src); c->src = nullptr; c->has_src = false;
+  cudaFree(c->gid); c->gid = nullptr; cudaFree(c->gid_new); c->gid_new = nullptr;
+  cudaFree(c->slot_of); c->slot_of = nullptr;
+  for (int k = 0; k < 3; ++k) { cudaFree(c->sflag[k]); c->sflag[k] = nullptr; cudaFree(c->stot[k]); c->stot[k] = nullptr; }
+  for (int k = 0; k < 2; ++k) { cudaFree(c->halo_list[k]); c->halo_list[k] = nullptr; }
+  cudaFree(c->mig_buf); c->mig_buf = nullptr;
   c->loaded = false;
 }
 
@@ -219,6 +241,7 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
                                                         c->orig[0], c->orig[1]);
     std::swap(c->Y[0], c->Y[1]);
     std::swap(c->orig[0], c->orig[1]);
+    c->inv_valid = false;
     Ycur = c->Y[0];
     iota_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.perm, N);
     c->launches += 2;
@@ -252,7 +275,8 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in)
   if ((rc = mark(c))) return rc;
   /* a5 */
   cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
-  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, c->tb, Ycur, np, c->so, c->status, rk_in.update);
+  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, c->tb, Ycur, np, c->so, c->status, rk_in.update, c->orig[0],
+                                               rk_in.n_own);
   if ((rc = mark(c))) return rc;
   /* a6 */
   launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
@@ -281,54 +305,55 @@ int substep(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk) {
   return rc;
 }
 
-int rk_step(ccake_ctx* c) {
-  const double dt = c->P.dx0, x0 = c->x0;
+/* substep k of the RK scheme (DESIGN reading 7).  RK2 midpoint: k1 = f(y0, x0); yh = y0 + dt/2 k1; k2 = f(yh, x0 + dt/2);
+   y1 = y0 + dt k2.  Classical RK4 with the accumulator Y[2].  Substep 0 reorders Y[0] into Y[1] and swaps, so "base" and
+   "out" are named after the swap; the last substep advances the time. */
+int rk_substep(ccake_ctx* c, int k) {
+  const double dt = c->P.dx0;
+  const bool rk2 = c->P.integrator == 2;
+  const int nsub = rk2 ? 2 : 4;
   int rc;
   RkArgs rk;
   std::memset(&rk, 0, sizeof(rk));
   rk.update = 1;
-  if (c->P.integrator == 2) {
-    /* midpoint (DESIGN reading 7): k1 = f(y0, x0); yh = y0 + dt/2 k1; k2 = f(yh, x0 + dt/2); y1 = y0 + dt k2.
-       The first substep reorders Y[0] into Y[1] and swaps, so "base" and "out" are named after the swap. */
-    rk.acc_mode = 0;
-    rk.c_out = 0.5 * dt;
-    rk.Ybase = nullptr; rk.Yout = nullptr;
-    {
-      double* Ycur = c->Y[0];
-      if ((rc = mark(c))) return rc;
-      if ((rc = build_cells(c, Ycur, true))) return rc;
-      if ((rc = mark(c))) return rc;
-      rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
-      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
-      if (rc) return rc;
-      if (c->timing) c->substeps_timed++;
-    }
-    rk.c_out = dt; rk.Ybase = c->Y[0]; rk.Yout = c->Y[0];
-    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
+  rk.n_own = c->slab ? c->n_own : c->N;
+  double off = 0.0;
+  if (k == 0) {
+    double* Ycur = c->Y[0];
+    if ((rc = mark(c))) return rc;
+    if ((rc = build_cells(c, Ycur, true))) return rc;
+    if ((rc = mark(c))) return rc;
+    rk.Ybase = c->Y[0]; rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt;
+    if (!rk2) { rk.Yacc = c->Y[2]; rk.acc_mode = 1; rk.w_acc = 1.0; }
+    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
+    if (rc) return rc;
+    if (c->timing) c->substeps_timed++;
   } else {
-    rk.Yacc = c->Y[2];
-    {
-      double* Ycur = c->Y[0];
-      if ((rc = mark(c))) return rc;
-      if ((rc = build_cells(c, Ycur, true))) return rc;
-      if ((rc = mark(c))) return rc;
-      rk.Ybase = c->Y[0]; rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt; rk.acc_mode = 1; rk.w_acc = 1.0;
-      rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
-      if (rc) return rc;
-      if (c->timing) c->substeps_timed++;
+    rk.Ybase = c->Y[0];
+    if (rk2) { rk.Yout = c->Y[0]; rk.c_out = dt; off = 0.5 * dt; }
+    else {
+      rk.Yacc = c->Y[2];
+      if (k == 1) { rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt; rk.acc_mode = 2; rk.w_acc = 2.0; off = 0.5 * dt; }
+      else if (k == 2) { rk.Yout = c->Y[1]; rk.c_out = dt; rk.acc_mode = 2; rk.w_acc = 2.0; off = 0.5 * dt; }
+      else { rk.Yout = c->Y[0]; rk.c_out = dt / 6.0; rk.acc_mode = 3; rk.w_acc = 2.0; off = dt; }
     }
-    rk.Ybase = c->Y[0]; rk.Yout = c->Y[1];
-    rk.c_out = 0.5 * dt; rk.acc_mode = 2; rk.w_acc = 2.0;
-    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
-    rk.c_out = dt;
-    if ((rc = substep(c, c->Y[1], 0.5 * dt, rk))) return rc;
-    rk.Yout = c->Y[0]; rk.c_out = dt / 6.0; rk.acc_mode = 3;
-    if ((rc = substep(c, c->Y[1], dt, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], off, rk))) return rc;
   }
-  advance_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, dt);      /* x0 <- x0 + dt, the same operation as on the host below */
-  c->launches += 1;
-  c->x0 = x0 + dt;
-  c->derived_valid = false;
+  if (k == nsub - 1) {
+    advance_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, dt);    /* x0 <- x0 + dt, the same operation as on the host below */
+    c->launches += 1;
+    c->x0 = c->x0 + dt;
+    c->derived_valid = false;
+  }
+  return CCAKE_OK;
+}
+
+int rk_step(ccake_ctx* c) {
+  const int nsub = (c->P.integrator == 2) ? 2 : 4;
+  for (int k = 0; k < nsub; ++k) {
+    const int rc = rk_substep(c, k);
+    if (rc) return rc;
+  }
   return CCAKE_OK;
 }
 
@@ -452,6 +477,7 @@ int refresh(ccake_ctx* c) {
   RkArgs rk;
   std::memset(&rk, 0, sizeof(rk));
   rk.update = 0;
+  rk.n_own = c->slab ? c->n_own : c->N;
   rk.Krate = c->Krate;
   if (!c->diag) CK(cudaMalloc(&c->diag, sizeof(double) * c->npad * 4));
   rk.diag = c->diag;
@@ -682,21 +708,23 @@ static int reload_particles(ccake_ctx* c, int32_t nfields, const int32_t* ids, c
   return launch_check(c, "reload");
 }
 
-int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* ids, const double* const* cols,
-                         int32_t memspace) {
-  if (!c) return CCAKE_EINVAL;
-  if (n <= 0 || nfields <= 0 || !ids || !cols || n > 2000000000LL || (memspace != 0 && memspace != 1)) {
-    c->err = "bad arguments to ccake_load_particles";
-    return CCAKE_EINVAL;
-  }
-  for (int k = 0; k < nfields; ++k)
-    if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in load"; return CCAKE_EINVAL; }
-  CK(cudaSetDevice(c->device));
-  CK(cudaStreamSynchronize(c->stream));
-  if (c->loaded && n == c->N) return reload_particles(c, nfields, ids, cols, memspace);
-  free_particles(c);
+/* sizes that follow the current particle count (a slab context changes it every step; the arrays are sized for the capacity) */
+static void set_count(ccake_ctx* c, int64_t n) {
   c->N = n;
-  c->npad = (n + 31) / 32 * 32;
+  c->bbox_blocks = std::min(nblk(n, BBOX_THREADS), 1024);
+  c->tot_blocks = std::min(nblk(n, TOT_THREADS), 1184);
+  c->ntiles = nblk(n, SORT_TILE);
+  c->hist_len = (int64_t)256 * c->ntiles;
+  c->nchunks = nblk(c->hist_len, SCAN_CHUNK);
+}
+
+/* n particles in arrays sized for cap >= n */
+static int load_impl(ccake_ctx* c, int64_t n, int64_t cap, int32_t nfields, const int32_t* ids, const double* const* cols,
+                     int32_t memspace) {
+  free_particles(c);
+  c->cap = cap;
+  c->N = n;
+  c->npad = (cap + 31) / 32 * 32;
   const int64_t np = c->npad;
   const int nbuf = (c->P.integrator == 4) ? 3 : 2;
   for (int k = 0; k < nbuf; ++k) {
@@ -714,7 +742,7 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
     /* hit-mask cache: MASK_TILES tiles per pair block, 16 B per group of 8 homes and tile; capped at 1/8 of the free
        memory and dropped altogether if the allocation fails — the gradient pass then culls for itself.  Test knobs
        (include/ccake.h): the environment variables CCAKE_MASK_TILES and CCAKE_CAND_CAP override the two sizes. */
-    const size_t nblocks = (size_t)((c->N + BH - 1) / BH), per_tile = sizeof(uint4) * NGRP;
+    const size_t nblocks = (size_t)((cap + BH - 1) / BH), per_tile = sizeof(uint4) * NGRP;
     size_t free_b = 0, total_b = 0;
     int tiles = MASK_TILES;
     if (const char* e = std::getenv("CCAKE_MASK_TILES")) tiles = std::max(0, std::atoi(e));
@@ -735,16 +763,13 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   CK(cudaMalloc(&c->nnb, sizeof(uint32_t) * np));
   CK(cudaMalloc(&c->theta, sizeof(double) * np));
   CK(cudaMalloc(&c->scratch, sizeof(double) * np));
-  c->bbox_blocks = std::min(nblk(n, BBOX_THREADS), 1024);
+  set_count(c, cap);
   CK(cudaMalloc(&c->bbox_partial, sizeof(double) * 6 * c->bbox_blocks));
-  c->tot_blocks = std::min(nblk(n, TOT_THREADS), 1184);
   CK(cudaMalloc(&c->tot_partial, sizeof(double) * TOT_NV * c->tot_blocks));
   CK(cudaMalloc(&c->tot_out, sizeof(double) * 16));
-  c->ntiles = nblk(n, SORT_TILE);
-  c->hist_len = (int64_t)256 * c->ntiles;
-  c->nchunks = nblk(c->hist_len, SCAN_CHUNK);
   CK(cudaMalloc(&c->hist, sizeof(uint32_t) * c->hist_len));
   CK(cudaMalloc(&c->chunk_tot, sizeof(uint32_t) * c->nchunks));
+  set_count(c, n);
   /* fields */
   fill_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->Y[0] + (int64_t)CCAKE_MASS * np, n, 1.0);
   for (int k = 0; k < nfields; ++k) {
@@ -779,6 +804,22 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   c->derived_valid = false;
   int rc = launch_check(c, "load");
   return rc;
+}
+
+int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* ids, const double* const* cols,
+                         int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (n <= 0 || nfields <= 0 || !ids || !cols || n > 2000000000LL || (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_load_particles";
+    return CCAKE_EINVAL;
+  }
+  for (int k = 0; k < nfields; ++k)
+    if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in load"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  if (c->loaded && !c->slab && n == c->N && c->cap == n) return reload_particles(c, nfields, ids, cols, memspace);
+  c->slab = false;
+  return load_impl(c, n, n, nfields, ids, cols, memspace);
 }
 
 int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4],
@@ -1047,10 +1088,261 @@ int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* cons
   return CCAKE_OK;
 }
 
+/* ============================================================ slab decomposition of one event (slab.cuh) ==== */
+namespace {
+const double SLAB_INF = 1.0e300;
+
+int slab_alloc(ccake_ctx* c) {
+  const int64_t cap = c->npad;
+  const int64_t nch = nblk(cap, SCAN_CHUNK) + 1;
+  CK(cudaMalloc(&c->gid, sizeof(uint32_t) * cap));
+  CK(cudaMalloc(&c->gid_new, sizeof(uint32_t) * cap));
+  CK(cudaMalloc(&c->slot_of, sizeof(uint32_t) * cap));
+  for (int k = 0; k < 3; ++k) {
+    CK(cudaMalloc(&c->sflag[k], sizeof(uint32_t) * cap));
+    CK(cudaMalloc(&c->stot[k], sizeof(uint32_t) * nch));
+  }
+  for (int k = 0; k < 2; ++k) CK(cudaMalloc(&c->halo_list[k], sizeof(uint32_t) * cap));
+  CK(cudaMalloc(&c->mig_buf, sizeof(double) * SLAB_NF * cap));
+  return CCAKE_OK;
+}
+
+/* exclusive ranks of the flags in sflag[k] (in place) + chunk offsets in stot[k] */
+void slab_scan(ccake_ctx* c, int k, int64_t n) {
+  const int nch = nblk(n, SCAN_CHUNK);
+  scan_chunk_kernel<<<nch, SCAN_CHUNK, 0, c->stream>>>(c->sflag[k], n, c->stot[k]);
+  scan_totals_kernel<<<1, 1024, 0, c->stream>>>(c->stot[k], nch);
+  c->launches += 2;
+}
+
+/* host copy of a device count (the message sizes steer the host: one small synchronous copy per message) */
+int slab_fetch_count(ccake_ctx* c, int64_t n, int cls, double lo_edge, double hi_edge, int k, int64_t* out) {
+  long long* d = reinterpret_cast<long long*>(c->tot_out);     /* 16 doubles of scratch */
+  slab_count_kernel<<<1, 1, 0, c->stream>>>(c->sflag[k], c->stot[k], n, c->Y[0], c->npad, c->slab_axis, lo_edge, hi_edge, c->orig[0],
+                                           c->n_own, cls, d);
+  long long h = 0;
+  CK(cudaMemcpyAsync(&h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  *out = (int64_t)h;
+  c->launches += 1;
+  return CCAKE_OK;
+}
+
+int slab_need(ccake_ctx* c, const char* what) {
+  if (!c->slab || !c->loaded) { c->err = std::string(what) + ": not a loaded slab context"; return CCAKE_ESTATE; }
+  return CCAKE_OK;
+}
+
+void slab_inverse(ccake_ctx* c) {
+  if (c->inv_valid) return;
+  slab_inverse_kernel<<<nblk(c->N, 256), 256, 0, c->stream>>>(c->orig[0], c->N, c->slot_of);
+  c->launches += 1;
+  c->inv_valid = true;
+}
+}  // namespace
+
+int ccake_slab_load(ccake_ctx* c, int64_t n_own, int64_t capacity, int32_t nfields, const int32_t* ids, const double* const* cols,
+                    const uint32_t* gids, int32_t axis, double lo, double hi, double halo_width, int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  if (n_own <= 0 || capacity < n_own || capacity > 2000000000LL || nfields <= 0 || !ids || !cols || axis < 0 || axis >= c->P.dim ||
+      !(lo < hi) || !(halo_width >= 0.0) || (memspace != 0 && memspace != 1)) {
+    c->err = "bad arguments to ccake_slab_load";
+    return CCAKE_EINVAL;
+  }
+  for (int k = 0; k < nfields; ++k)
+    if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in load"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  int rc = load_impl(c, n_own, capacity, nfields, ids, cols, memspace);
+  if (rc) return rc;
+  if ((rc = slab_alloc(c))) return rc;
+  c->slab = true;
+  c->slab_axis = axis; c->slab_lo = lo; c->slab_hi = hi; c->slab_w = halo_width;
+  c->n_own = n_own;
+  c->n_ghost[0] = c->n_ghost[1] = 0; c->halo_cnt[0] = c->halo_cnt[1] = 0; c->mig_in[0] = c->mig_in[1] = 0;
+  c->inv_valid = false;
+  if (gids) CK(cudaMemcpyAsync(c->gid, gids, sizeof(uint32_t) * n_own, memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
+  else slab_iota_gid_kernel<<<nblk(n_own, 256), 256, 0, c->stream>>>(c->gid, n_own, 0u);
+  CK(cudaStreamSynchronize(c->stream));
+  return launch_check(c, "slab_load");
+}
+
+int ccake_slab_export_halo(ccake_ctx* c, int32_t side, int32_t k, double* buf, int64_t buf_cap, int64_t* count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_export_halo");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || k < 0 || !buf || buf_cap <= 0 || !count) { c->err = "bad arguments to ccake_slab_export_halo"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = c->stream;
+  const int64_t N = c->N, np = c->npad;
+  if (k == 0) {
+    /* owned particles within halo_width of the face, in store order; the list of their load indices serves the later substeps */
+    /* one face at a time: in a slab thinner than 2 halo_width a particle belongs to both halos */
+    const double lo_edge = (side != 0 || c->slab_lo <= -SLAB_INF) ? -SLAB_INF : c->slab_lo + c->slab_w;
+    const double hi_edge = (side != 1 || c->slab_hi >= SLAB_INF) ? SLAB_INF : c->slab_hi - c->slab_w;
+    const int cls = 1 + side, ks = 1 + side;
+    slab_flag_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->slab_axis, lo_edge, hi_edge, c->orig[0], c->n_own, nullptr,
+                                                   side == 0 ? c->sflag[ks] : nullptr, side == 1 ? c->sflag[ks] : nullptr);
+    slab_scan(c, ks, N);
+    int64_t cnt = 0;
+    if ((rc = slab_fetch_count(c, N, cls, lo_edge, hi_edge, ks, &cnt))) return rc;
+    *count = cnt;
+    if (cnt > buf_cap) { c->err = "halo message larger than the buffer"; return CCAKE_ENOMEM; }
+    if (cnt > 0)
+      slab_pack_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->slab_axis, lo_edge, hi_edge, c->orig[0], c->n_own, cls, c->sflag[ks],
+                                                     c->stot[ks], c->gid, buf, buf_cap, c->halo_list[side]);
+    c->halo_cnt[side] = cnt;
+    c->launches += 2;
+  } else {
+    const int64_t cnt = c->halo_cnt[side];
+    *count = cnt;
+    if (cnt > buf_cap) { c->err = "halo message larger than the buffer"; return CCAKE_ENOMEM; }
+    slab_inverse(c);
+    if (cnt > 0)
+      slab_repack_kernel<<<nblk(cnt, 256), 256, 0, st>>>(c->Y[1], np, cnt, c->halo_list[side], c->slot_of, c->gid, buf, buf_cap);
+    c->launches += 1;
+  }
+  return launch_check(c, "slab_export_halo");
+}
+
+int ccake_slab_import_ghosts(ccake_ctx* c, int32_t side, int32_t k, const double* buf, int64_t buf_cap, int64_t count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_import_ghosts");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || k < 0 || count < 0 || (count > 0 && !buf) || buf_cap < count) { c->err = "bad arguments to ccake_slab_import_ghosts"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = c->stream;
+  const int64_t np = c->npad;
+  if (k == 0) {
+    if (c->N + count > c->cap) { c->err = "ghosts exceed the capacity of the slab context"; return CCAKE_ENOMEM; }
+    /* the low side's ghosts take the load indices right behind the owned particles, the high side's follow */
+    if (side == 0 && c->n_ghost[1] > 0) { c->err = "import the low side's ghosts before the high side's"; return CCAKE_ESTATE; }
+    if (c->n_ghost[side] > 0) { c->err = "the ghosts of an earlier exchange are still there: ccake_slab_commit first"; return CCAKE_ESTATE; }
+    const int64_t load0 = c->n_own + (side == 0 ? 0 : c->n_ghost[0]);
+    if (count > 0)
+      slab_append_kernel<<<nblk(count, 256), 256, 0, st>>>(c->Y[0], np, c->N, load0, count, buf, buf_cap, c->orig[0], c->gid);
+    c->n_ghost[side] = count;
+    set_count(c, c->N + count);
+    c->inv_valid = false;
+    c->derived_valid = false;
+  } else {
+    if (count != c->n_ghost[side]) { c->err = "ghost message of a later substep differs in size from the first"; return CCAKE_EINVAL; }
+    slab_inverse(c);
+    const int64_t load0 = c->n_own + (side == 0 ? 0 : c->n_ghost[0]);
+    if (count > 0) slab_refresh_kernel<<<nblk(count, 256), 256, 0, st>>>(c->Y[1], np, load0, count, buf, buf_cap, c->slot_of);
+  }
+  c->launches += 1;
+  return launch_check(c, "slab_import_ghosts");
+}
+
+int ccake_slab_substep(ccake_ctx* c, int32_t k) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_substep");
+  if (rc) return rc;
+  const int nsub = (c->P.integrator == 2) ? 2 : 4;
+  if (k < 0 || k >= nsub) { c->err = "substep index out of range"; return CCAKE_EINVAL; }
+  if (c->P.eos_kind == 1 && !c->table_loaded) { c->err = "step before table load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  rc = rk_substep(c, k);
+  if (k == 0) c->inv_valid = false;            /* the store was reordered */
+  return rc;
+}
+
+int ccake_slab_export_migrants(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_export_migrants");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || !buf || buf_cap <= 0 || !count) { c->err = "bad arguments to ccake_slab_export_migrants"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = c->stream;
+  const int64_t N = c->N, np = c->npad;
+  const int cls = 1 + side, ks = 1 + side;
+  slab_flag_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->slab_axis, c->slab_lo, c->slab_hi, c->orig[0], c->n_own, nullptr,
+                                                 side == 0 ? c->sflag[ks] : nullptr, side == 1 ? c->sflag[ks] : nullptr);
+  slab_scan(c, ks, N);
+  int64_t cnt = 0;
+  if ((rc = slab_fetch_count(c, N, cls, c->slab_lo, c->slab_hi, ks, &cnt))) return rc;
+  *count = cnt;
+  if (cnt > buf_cap) { c->err = "migrant message larger than the buffer"; return CCAKE_ENOMEM; }
+  if (cnt > 0)
+    slab_pack_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->slab_axis, c->slab_lo, c->slab_hi, c->orig[0], c->n_own, cls, c->sflag[ks],
+                                                   c->stot[ks], c->gid, buf, buf_cap, nullptr);
+  c->launches += 2;
+  return launch_check(c, "slab_export_migrants");
+}
+
+int ccake_slab_import_migrants(ccake_ctx* c, int32_t side, const double* buf, int64_t buf_cap, int64_t count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_import_migrants");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || count < 0 || (count > 0 && !buf) || buf_cap < count || count > c->npad / 2) { c->err = "bad arguments to ccake_slab_import_migrants"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  if (count > 0)
+    slab_park_kernel<<<nblk(count, 256), 256, 0, c->stream>>>(buf, buf_cap, count, c->mig_buf, c->npad, side == 0 ? 0 : c->npad / 2);
+  c->mig_in[side] = count;
+  c->launches += 1;
+  return launch_check(c, "slab_import_migrants");
+}
+
+int ccake_slab_commit(ccake_ctx* c, int64_t* n_own_new) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_commit");
+  if (rc) return rc;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = c->stream;
+  const int64_t N = c->N, np = c->npad;
+  /* the owned particles still inside [lo, hi), compacted in store order into Y[1] (free at the end of a step) */
+  slab_flag_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], np, N, c->slab_axis, c->slab_lo, c->slab_hi, c->orig[0], c->n_own, c->sflag[0], nullptr, nullptr);
+  slab_scan(c, 0, N);
+  int64_t nstay = 0;
+  if ((rc = slab_fetch_count(c, N, 0, c->slab_lo, c->slab_hi, 0, &nstay))) return rc;
+  const int64_t nnew = nstay + c->mig_in[0] + c->mig_in[1];
+  if (nnew > c->cap) { c->err = "owned particles exceed the capacity of the slab context"; return CCAKE_ENOMEM; }
+  if (nnew <= 0) { c->err = "a slab ran empty"; return CCAKE_ERANGE; }
+  CK(cudaMemsetAsync(c->Y[1], 0, sizeof(double) * np * NSTATE, st));
+  slab_keep_kernel<<<nblk(N, 256), 256, 0, st>>>(c->Y[0], c->Y[1], np, N, c->slab_axis, c->slab_lo, c->slab_hi, c->orig[0], c->n_own, c->sflag[0],
+                                                 c->stot[0], c->gid, c->gid_new);
+  int64_t at = nstay;
+  for (int sd = 0; sd < 2; ++sd) {
+    if (c->mig_in[sd] > 0)
+      slab_arrive_kernel<<<nblk(c->mig_in[sd], 256), 256, 0, st>>>(c->Y[1], np, at, c->mig_in[sd], c->mig_buf, np, sd == 0 ? 0 : np / 2, c->gid_new);
+    at += c->mig_in[sd];
+  }
+  std::swap(c->Y[0], c->Y[1]);
+  std::swap(c->gid, c->gid_new);
+  iota_kernel<<<nblk(nnew, 256), 256, 0, st>>>(c->orig[0], nnew);
+  c->launches += 5;
+  c->n_own = nnew;
+  set_count(c, nnew);
+  c->n_ghost[0] = c->n_ghost[1] = 0; c->halo_cnt[0] = c->halo_cnt[1] = 0; c->mig_in[0] = c->mig_in[1] = 0;
+  c->inv_valid = false;
+  c->derived_valid = false;
+  if (n_own_new) *n_own_new = nnew;
+  return launch_check(c, "slab_commit");
+}
+
+int ccake_slab_info(ccake_ctx* c, int64_t out[4]) {
+  if (!c || !out) return CCAKE_EINVAL;
+  out[0] = c->slab ? c->n_own : c->N; out[1] = c->n_ghost[0]; out[2] = c->n_ghost[1]; out[3] = c->cap;
+  return CCAKE_OK;
+}
+
+int ccake_slab_gids(ccake_ctx* c, uint32_t* out, int64_t capacity, int32_t memspace) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_gids");
+  if (rc) return rc;
+  if (!out || capacity < c->N || (memspace != 0 && memspace != 1)) { c->err = "bad arguments to ccake_slab_gids"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaMemcpyAsync(out, c->gid, sizeof(uint32_t) * c->N, memspace == CCAKE_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return CCAKE_OK;
+}
+
 int ccake_step(ccake_ctx* c, int32_t nsteps) {
   if (!c) return CCAKE_EINVAL;
   if (nsteps < 0) { c->err = "nsteps < 0"; return CCAKE_EINVAL; }
   if (!c->loaded || (c->P.eos_kind == 1 && !c->table_loaded)) { c->err = "step before load"; return CCAKE_ESTATE; }
+  if (c->slab) { c->err = "a slab context is stepped substep by substep (ccake_slab_substep)"; return CCAKE_ESTATE; }
   CK(cudaSetDevice(c->device));
   for (int s = 0; s < nsteps; ++s) {
     if (!c->use_graphs || c->timing) {              /* per-kernel timing needs the events between the launches */
@@ -1205,7 +1497,8 @@ int ccake_conserved_totals(ccake_ctx* c, double out[16]) {
   int rc = refresh(c);
   if (rc) return rc;
   const Geom gm = make_geom(c->P.coords, c->x0);
-  totals_partial_kernel<<<c->tot_blocks, TOT_THREADS, 0, c->stream>>>(c->N, c->kp, gm, c->Y[0], c->npad, c->so, c->tot_partial);
+  totals_partial_kernel<<<c->tot_blocks, TOT_THREADS, 0, c->stream>>>(c->N, c->kp, gm, c->Y[0], c->npad, c->so, c->tot_partial, c->orig[0],
+                                                                     c->slab ? c->n_own : c->N);
   totals_final_kernel<<<1, 32, 0, c->stream>>>(c->tot_partial, c->tot_blocks, c->tot_out);
   if ((rc = launch_check(c, "totals"))) return rc;
   double t[TOT_NV];

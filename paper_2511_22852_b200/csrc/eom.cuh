@@ -260,7 +260,9 @@ struct RkArgs {
   double* theta_out;    /* sorted order                            */
   double* diag;         /* 4 x npad, sorted order: Kn_pi, Re_pi^-1, Kn_Pi, Re_Pi^-1 (DIAG kernels only) */
   const double* src;    /* 7 x npad, ORIGINAL particle order: I^0..I^3, I_B, I_S, I_Q (ccake_set_sources), or NULL */
-  const uint32_t* orig; /* store slot -> original index (for src)  */
+  const uint32_t* orig; /* store slot -> original (load) index: for src, and to tell ghosts */
+  int64_t n_own;        /* load indices >= n_own are ghost particles of a slab context (slab.cuh): evolved like the rest, but
+                           their rates are not valid and not checked (their state is re-imported before every substep) */
   double c_out, w_acc;
   int acc_mode;         /* 0 none | 1 set | 2 add | 3 final        */
   int update;           /* 0: rates only (refresh)                 */
@@ -469,7 +471,7 @@ eom_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_o
     rk.diag[2 * npad + i] = in.tau_Pi * o.theta;
     rk.diag[3 * npad + i] = fabs(in.ds.bulkt * in.sig) / in.p;
   }
-  if (!ok || !(o.dS == o.dS) || !(du[0] == du[0])) atomicAdd(&status->n_bad, 1ULL);
+  if ((!ok || !(o.dS == o.dS) || !(du[0] == du[0])) && (int64_t)rk.orig[a] < rk.n_own) atomicAdd(&status->n_bad, 1ULL);
 
   /* rates of the evolved set */
   double k_[NSTATE];

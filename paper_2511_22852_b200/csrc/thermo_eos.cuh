@@ -455,7 +455,7 @@ __device__ inline void load_u(const KParams& kp, const Geom& gm, const double* Y
 
 __global__ void __launch_bounds__(128)
 thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_off, TableDev tb, const double* __restrict__ Y,
-              int64_t npad, Sorted so, Status* __restrict__ status, int on_step) {
+              int64_t npad, Sorted so, Status* __restrict__ status, int on_step, const uint32_t* __restrict__ orig, int64_t n_own) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const Geom gm = make_geom(kp.coords, *x0_dev + x0_off);      /* the time lives on the device: a captured step replays */
@@ -470,7 +470,8 @@ thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x
   double nq[NQ];
   for (int q = 0; q < NQ; ++q) nq[q] = so.rho_star[q][i] / lab;
   const ThermoOut th = (kp.eos_kind == 0) ? eos_closed_form(kp, s, nq) : eos_table_lookup(tb, s, nq);
-  if (th.oob) {                       /* clamped to the table: latest pass, and all substeps of steps since the load */
+  if (th.oob && (int64_t)orig[a] < n_own) {   /* clamped to the table (ghosts of a slab context, whose sums are incomplete, do
+                                                  not count): latest pass, and all substeps of steps since the load */
     atomicAdd(&status->n_oob, 1ULL);
     if (on_step) atomicAdd(&status->n_oob_total, 1ULL);
   }

@@ -16,12 +16,13 @@ constexpr int TOT_NV = 14;   /* E, P1..3, S, NB, NS, NQ, M, work, npairs, (unuse
 
 __global__ void __launch_bounds__(TOT_THREADS)
 totals_partial_kernel(int64_t n, KParams kp, Geom gm, const double* __restrict__ Y, int64_t npad, Sorted so,
-                      double* __restrict__ partial) {
+                      double* __restrict__ partial, const uint32_t* __restrict__ orig, int64_t n_own) {
   double acc[TOT_NV];
   for (int k = 0; k < TOT_NV; ++k) acc[k] = 0.0;
   const int D = kp.D;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     const int64_t a = so.perm[i];
+    if ((int64_t)orig[a] >= n_own) continue;        /* ghost of a slab context: counted by its owner */
     double u[4];
     load_u(kp, gm, Y, npad, a, u);
     const double gam = u[0], sig = so.sigma[i], m = Y[CCAKE_MASS * npad + a];
