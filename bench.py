@@ -73,18 +73,25 @@ def shared_table():
     return _TABLES["t"]
 
 
-def make_workload(name, rank=0, tiles=None):
+def make_workload(name, rank=0, tiles=None, world=1):
+    """Workload of one rank: rank r of `world` evolves the event tiles sharding.tile_range gives it (weak scaling: every rank
+    the same number of tiles, seeds by global tile number)."""
     from paper_2511_22852_b200 import workloads as W
+    from paper_2511_22852_b200 import sharding
+    world = max(world, rank + 1)
+
+    def first_tile(per_rank):
+        return sharding.tile_range(per_rank * world, rank, world).start
     if name == "C1":
         return W.config_c1()
     if name == "C2":
         return W.config_c2()
     if name == "C3":
-        return W.config_c3(tile0=4 * rank, table=shared_table())
+        return W.config_c3(tile0=first_tile(4), table=shared_table())
     if name == "C4":
-        return W.config_c4(K=tiles or 10, tile0=10 * rank, table=shared_table())
+        return W.config_c4(K=tiles or 10, tile0=first_tile(tiles or 10), table=shared_table())
     if name == "C5":
-        return W.config_c5(tile0=13 * rank)
+        return W.config_c5(tile0=first_tile(13))
     if name == "C4p":
         return W.config_c4p(table=shared_table())
     raise SystemExit(f"unknown config {name}")
@@ -271,6 +278,123 @@ def short_run(name, steps, device, hbm):
             "rc": rc}
 
 
+def slab_probe(device, steps=5):
+    """One C4 event (198,400 particles, 80 x 80 x 31) as a single context and as 2 slabs cut in x on the SAME GPU (the slabs
+    run one after the other, so this measures what the decomposition costs — ghost recomputation, packing, the hand-over of
+    the messages — not a speed-up): ms per RK2 step each, ghosts per slab, message bytes per step."""
+    import torch
+    from paper_2511_22852_b200 import binding as B
+    from paper_2511_22852_b200 import sharding as S
+    w = make_workload("C4", tiles=1)
+    p = w.params
+    dev = torch.device("cuda", device)
+    stream = torch.cuda.Stream()
+    tab = torch.as_tensor(w.table["data"], device=dev)
+
+    def ctx():
+        g = B.Ccake(device=device, stream=stream.cuda_stream, **p)
+        g.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], tab)
+        return g
+
+    def timed(fn):
+        fn(2)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record()
+            fn(steps)
+            e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    one = ctx()
+    one.load_particles(w.fields)
+    ms_one = timed(one.step)
+    one.close()
+    axis, K = 0, 2
+    planes = S.slab_planes(w.fields[B.R1 + axis], K)
+    width = S.slab_halo_width(p["h"], p["dx0"])
+    slabs = {}
+    for k in range(K):
+        lo, hi = S.slab_bounds(planes, k)
+        sel = np.nonzero((w.fields[B.R1 + axis] >= lo) & (w.fields[B.R1 + axis] < hi))[0]
+        g = ctx()
+        g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), int(0.9 * w.n), axis, lo, hi, width)
+        slabs[k] = g
+    drv = S.SlabDriver(slabs, K, 2, int(0.5 * w.n), lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev))
+    with torch.cuda.stream(stream):
+        ms_slabs = timed(drv.step)
+        b0 = drv.bytes_moved
+        drv.step(1)
+        per_step = drv.bytes_moved - b0
+        drv.refresh_ghosts()
+    info = [g.slab_info() for g in slabs.values()]
+    for g in slabs.values():
+        g.close()
+    return {"event_particles": w.n, "slabs": K, "axis": "x", "halo_width_fm": width, "ms_per_step_one_context": ms_one,
+            "ms_per_step_slabs_same_gpu": ms_slabs, "owned_per_slab": [i[0] for i in info], "ghosts_per_slab": [i[1] + i[2] for i in info],
+            "message_bytes_per_step": per_step,
+            "note": "2 contexts on one GPU, run one after the other: the cost of the decomposition, not a scaling number"}
+
+
+def run_slabs(args):
+    """--decomp slabs: ONE event (C4, a single tile of 198,400 particles) cut into one slab per rank along x; halos and
+    migrants travel by torch.distributed send / recv (NCCL).  value = particles of the event x steps / device time (max
+    over ranks): strong scaling of one event."""
+    import torch
+    import torch.distributed as dist
+    from paper_2511_22852_b200 import binding as B
+    from paper_2511_22852_b200 import sharding as S
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    w = make_workload("C4", tiles=1)
+    p = w.params
+    K = max(world, 2) if world == 1 else world
+    axis = 0
+    planes = S.slab_planes(w.fields[B.R1 + axis], K)
+    width = S.slab_halo_width(p["h"], p["dx0"])
+    stream = torch.cuda.Stream()
+    tab = torch.as_tensor(w.table["data"], device=dev)
+    slabs = {}
+    for k in S.tile_range(K, rank, world):
+        lo, hi = S.slab_bounds(planes, k)
+        sel = np.nonzero((w.fields[B.R1 + axis] >= lo) & (w.fields[B.R1 + axis] < hi))[0]
+        g = B.Ccake(device=local, stream=stream.cuda_stream, **p)
+        g.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], tab)
+        g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), w.n, axis, lo, hi, width)
+        slabs[k] = g
+    drv = S.SlabDriver(slabs, K, 2, w.n // 2, lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev), rank=rank, world=world)
+    with torch.cuda.stream(stream):
+        drv.step(max(args.warmup, 3))
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        drv.step(args.steps)
+        e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = S.reduce_max(e0.elapsed_time(e1), dev)
+    launches = sum(g.launch_count() for g in slabs.values())
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": w.n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": "one C4 event (80 x 80 x 31 = 198,400 particles) cut into %d slabs along x, halo %.2f fm" % (K, width),
+                                     "decomposition": "slabs", "slabs": K}, "gpu_launches": launches}), flush=True)
+    for g in slabs.values():
+        g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -286,7 +410,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()   # fails loudly when libccake.so is missing
 
-    w = make_workload(args.config, rank=rank, tiles=args.tiles)
+    w = make_workload(args.config, rank=rank, tiles=args.tiles, world=world)
     p = w.params
     D = p["dim"]
     visc, bulk, diff = bool(p["flags"] & 1) and p["eom"] != 0, bool(p["flags"] & 2) and p["eom"] != 0, bool(p["flags"] & 4) and p["eom"] != 0
@@ -312,7 +436,6 @@ def run_ours(args):
         sim.step(1)
     sim.synchronize(strict=False)
     sim.load_particles(dfields)       # timed steps start from the loaded state, inputs resident in HBM
-    sim.enable_timing(True)
     sim.launch_count()
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
@@ -320,16 +443,24 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         e0.record()
         for _ in range(args.steps):
-            sim.step(1)
+            sim.step(1)               # the library replays its captured RK step (one CUDA graph per step)
         e1.record()
     torch.cuda.synchronize()
     barrier()
     clocks = sampler.stop() if sampler else None
     ms_total = e0.elapsed_time(e1)
     launches = sim.launch_count()
+    rc = sim.synchronize(strict=False)
+    # the same K steps once more from the loaded state with the library's per-kernel CUDA events (which need the kernels
+    # launched one by one): the per-kernel durations behind `kernels` and `roofline`
+    sim.load_particles(dfields)
+    sim.enable_timing(True)
+    with torch.cuda.stream(stream):
+        for _ in range(args.steps):
+            sim.step(1)
     kt = sim.kernel_times()           # per-substep averages of each kernel group, CUDA events on the same stream
     sim.enable_timing(False)
-    rc = sim.synchronize(strict=False)
+    sim.synchronize(strict=False)
     from paper_2511_22852_b200 import sharding
     ms_total = sharding.reduce_max(ms_total, dev)                 # max over ranks of the device time
     tot_n = torch.tensor([float(w.n)], dtype=torch.float64, device=dev)
@@ -500,6 +631,7 @@ def run_ours(args):
             "source_smearing": {"partons": 2000, "h_source": 1.4, "ms": src_ms,
                                 "note": "ccake_smear_sources through host buffers, incl. 63 MB device-to-host"},
             "other_configs": others,
+            "slab_decomposition": slab_probe(local) if (not args.no_others and world == 1) else None,
             "clocks": clocks,
             "status": {"rc": rc, "n_out_of_table": totals[11], "n_bad": totals[13], "x0": totals[0]},
         }
@@ -517,12 +649,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tiles", type=int, default=None, help="C4 only: number of event tiles (profiling runs; default 10)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--decomp", default="events", choices=["events", "slabs"],
+                    help="events: every rank evolves its own event tiles (default, weak scaling); slabs: ONE event cut into one slab per rank")
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs (other_configs)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp == "slabs":
+        run_slabs(args)
     else:
         run_ours(args)
 
