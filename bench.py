@@ -52,14 +52,18 @@ FP64_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12   # 148 SMs x 4 sub-part
 
 def ncu_traffic(config, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of a pair kernel, read from the committed ncu --set full
-    summary of this round (profiles/r2_traffic.json: written from the capture, with the command that made it); None
-    when the file has no entry for this workload — never a constant pasted into this script."""
-    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    summary of this round (profiles/r2_traffic.txt: lines "config kernel bytes", written from the capture named in
+    profiles/r2_README.md); None when the file has no entry for this workload — never a constant pasted into this script."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.txt")
     try:
         with open(p) as fh:
-            return json.load(fh).get(config, {}).get(kernel)
+            for line in fh:
+                t = line.split()
+                if len(t) == 3 and t[0] == config and t[1] == kernel:
+                    return float(t[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 _TABLES = {}
