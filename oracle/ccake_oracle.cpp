@@ -19,6 +19,8 @@
  *                                         uniform fluid, Bjorken ODE with a source, energy balance of a moving fluid,
  *                                         exact momentum / charge balance)
  *   extra   freeze-out surface element    Eq. 145-148 :1466-1482 (d_mu eps, n_mu, |d sigma|; pinned on Bjorken, Gubser)
+ *   extra   offline inverter, forward table :576-593, DESIGN reading 21 (pinned: affine map vs a linear solve, an independent
+ *                                         multilinear interpolator, second-order convergence to the exact inversion, backup EoS)
  *
  * There is no blocking, fusion or reordering: loops are gather form (for a { for b }), the per-particle linear
  * system in the unknown time derivatives is written LITERALLY in covariant form with generic 4x4 metric and
