@@ -170,7 +170,7 @@ int mark(ccake_ctx* c) {
 }
 
 /* layout of the sorted-order arena, in units of npad doubles */
-constexpr int ARENA_FIELDS = 3 + 2 + 8 + 5 + 6 + 11 + 32 + 3 + 3 + 3 + 9 + 9 + 1;
+constexpr int ARENA_FIELDS = 3 + 2 + 8 + 5 + 6 + 11 + GREC_D + 3 + 3 + 3 + 9 + 9 + 1;
 
 void carve(ccake_ctx* c) {
   Sorted& s = c->so;
@@ -188,7 +188,7 @@ void carve(ccake_ctx* c) {
   for (int q = 0; q < NQ; ++q) s.mu[q] = take();
   s.p = take(); s.e = take(); s.cs2 = take(); s.ws = take();
   for (int q = 0; q < NQ; ++q) s.wq[q] = take();
-  s.rec_g = take(32);
+  s.rec_g = take(GREC_D);
   for (int k = 0; k < 3; ++k) s.FP[k] = take();
   for (int k = 0; k < 3; ++k) s.FB[k] = take();
   for (int q = 0; q < NQ; ++q) s.FK[q] = take();

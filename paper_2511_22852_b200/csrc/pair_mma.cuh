@@ -151,8 +151,10 @@ struct PairGeom {
 };
 
 /* An operator describes one pass:
-     NREC         doubles per staged record (even); elements 0..D-1 are the position; every payload element is
-                  already multiplied by the SPH weight m_b of its particle, and element oM is m_b itself
+     NREC         doubles per staged record (even); elements 0, 1, 2 are the position (z = 0 in 2-D); every payload element
+                  is already multiplied by the SPH weight m_b of its particle
+     GIDMAJOR     the record stores the 4 operands of MMA column n contiguously at double 4 + 4 n (gradient pass); otherwise
+                  column n of tile T for weight j is element elem(T, j, n) (one 8-byte load each)
      NJ           pair weights per (home, b): 1 (W) or D (the components of grad W)
      NT           MMA column tiles: the pass accumulates NT * NJ matrices of 8 homes x 8 columns
      elem(T,j,n)  record element that is column n of tile T for weight j; ELEM_NONE = unused column
@@ -167,7 +169,7 @@ template <int D_, bool HASH_ = false>
 struct SmoothOp {
   static constexpr int D = D_;
   static constexpr bool HASH = HASH_;
-  static constexpr bool COUNT = true;
+  static constexpr bool COUNT = true, GIDMAJOR = false;
   static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3;
   static constexpr int elem(int, int, int n) { return (n <= 4) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
@@ -190,47 +192,98 @@ struct SmoothOp {
 };
 
 /* ------------------------------------------------------------------------------------------ a6 operator ---- */
-/* record layout of the gradient pass (written by the thermo kernel): x[D], m, then m times each of
-   P, u[D], v[D], B[D*D], K[3*D], alpha[3] */
-struct GLayout { int M, P, U, V, B, K, AL, NREC; };
-__host__ __device__ inline GLayout make_glayout(int D, bool visc, bool diff) {
-  GLayout g;
-  g.M = D; g.P = D + 1; g.U = D + 2; g.V = 2 * D + 2; g.B = 3 * D + 2;
+/* Quantities of the gradient pass, numbered as "elements": m, then m times each of P, u[D], v[D], B[D*D], K[3*D],
+   alpha[3] (written by the thermo kernel). */
+struct GLayout { int M, P, U, V, B, K, AL, N; };
+__host__ __device__ constexpr GLayout make_glayout(int D, bool visc, bool diff) {
+  GLayout g{};
+  g.M = 0; g.P = 1; g.U = 2; g.V = 2 + D; g.B = 2 + 2 * D;
   g.K = g.B + (visc ? D * D : 0);
   g.AL = g.K + (diff ? 3 * D : 0);
-  const int n0 = g.AL + (diff ? 3 : 0);
-  g.NREC = (n0 + 1) / 2 * 2;
+  g.N = g.AL + (diff ? 3 : 0);
   return g;
 }
-
 /* Column tiles (weight j = component of grad W):
      tile 0:  m | m P | m u_1..u_D | m alpha_B, alpha_S, alpha_Q (DIFF)       -> G_j, FP_j, DU_jk, DA_qj
               ( ideal fluid: | m v_j instead, so that one tile is enough )
-     tile 1:  m v_j | m B_j1..B_jD (VISC) | m K_Bj, K_Sj, K_Qj (DIFF)          -> div v, FB_k, FK_q (summed over j at the end) */
+     tile 1:  m v_j | m B_j1..B_jD (VISC) | m K_Bj, K_Sj, K_Qj (DIFF)          -> div v, FB_k, FK_q (summed over j at the end)
+   grad_elem = element in column n of tile T for weight j. */
+__host__ __device__ constexpr int grad_elem(int D, bool visc, bool diff, int T, int j, int n) {
+  const GLayout L = make_glayout(D, visc, diff);
+  const int NT = (visc || diff) ? 2 : 1;
+  const int cDU = 2, cDA = 2 + D, cFB = 1, cFK = 1 + (visc ? D : 0);
+  if (T == 0) {
+    if (n == 0) return L.M;
+    if (n == 1) return L.P;
+    if (n < cDU + D) return L.U + (n - cDU);
+    if (diff) return (n < cDA + 3) ? L.AL + (n - cDA) : ELEM_NONE;
+    if (NT == 1 && n == 2 + D) return L.V + j;
+    return ELEM_NONE;
+  }
+  if (n == 0) return L.V + j;
+  if (visc && n >= cFB && n < cFB + D) return L.B + j * D + (n - cFB);
+  if (diff && n >= cFK && n < cFK + 3) return L.K + (n - cFK) * D + j;
+  return ELEM_NONE;
+}
+/* Record (36 doubles): x, y, z, 0, then 8 blocks of 4 doubles, block n = the operands of MMA column n ("gid-major": the 4
+   operands of lane (gid, tig) are 32 contiguous bytes, two 16-byte loads from one address): slot 0 = column n of tile 0,
+   slots 1..3 = column n of tile 1 for j = 0, 1, 2 (viscous / diffusive), or slots 0..2 = column n of the single tile for
+   j = 0, 1, 2 (ideal fluid: only its v_j column depends on j). */
+constexpr int GREC_D = 36, GREC_B0 = 4;
+__host__ __device__ constexpr int grad_slot_elem(int D, bool visc, bool diff, int n, int s) {
+  const bool two = visc || diff;
+  const int T = two ? (s == 0 ? 0 : 1) : 0;
+  const int j = two ? (s == 0 ? 0 : s - 1) : s;
+  if (j >= D) return ELEM_NONE;
+  return grad_elem(D, visc, diff, T, j, n);
+}
+/* position (double index in the record) of element e: its first appearance in the blocks */
+__host__ __device__ constexpr int grad_pos(int D, bool visc, bool diff, int e) {
+  for (int n = 0; n < 8; ++n)
+    for (int s = 0; s < 4; ++s)
+      if (grad_slot_elem(D, visc, diff, n, s) == e) return GREC_B0 + 4 * n + s;
+  return -1;
+}
+/* thermo kernel: scatter the elements el[0 .. L.N) of one particle into its record */
+template <int D, bool VISC, bool DIFF>
+__device__ __forceinline__ void write_grad_record(double* __restrict__ rg, const double* el) {
+#pragma unroll
+  for (int n = 0; n < 8; ++n) {
+    double v[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const int e = grad_slot_elem(D, VISC, DIFF, n, s);
+      v[s] = (e >= 0) ? el[e] : 0.0;
+    }
+    reinterpret_cast<double2*>(rg + GREC_B0 + 4 * n)[0] = make_double2(v[0], v[1]);
+    reinterpret_cast<double2*>(rg + GREC_B0 + 4 * n)[1] = make_double2(v[2], v[3]);
+  }
+}
+
 template <int D_, bool VISC, bool DIFF>
 struct GradOp {
   static constexpr int D = D_;
-  static constexpr bool HASH = false, COUNT = false;
-  static constexpr int oM = D, oP = D + 1, oU = D + 2, oV = 2 * D + 2, oB = 3 * D + 2;
-  static constexpr int oK = oB + (VISC ? D * D : 0), oAL = oK + (DIFF ? 3 * D : 0);
-  static constexpr int NREC = (oAL + (DIFF ? 3 : 0) + 1) / 2 * 2;
+  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = true;
+  static constexpr int eM = make_glayout(D_, VISC, DIFF).M, eP = make_glayout(D_, VISC, DIFF).P, eU = make_glayout(D_, VISC, DIFF).U,
+                       eV = make_glayout(D_, VISC, DIFF).V, eB = make_glayout(D_, VISC, DIFF).B, eK = make_glayout(D_, VISC, DIFF).K,
+                       eAL = make_glayout(D_, VISC, DIFF).AL;
+  static constexpr int NREC = GREC_D;
   static constexpr int NJ = D, NT = (VISC || DIFF) ? 2 : 1;
+  static constexpr int elem(int, int, int) { return ELEM_NONE; }       /* not used: the operands are found by position */
   /* column positions */
   static constexpr int cG = 0, cFP = 1, cDU = 2, cDA = 2 + D;
   static constexpr int tDV = NT - 1, cDV = (NT == 2) ? 0 : 2 + D, cFB = 1, cFK = 1 + (VISC ? D : 0);
-  static constexpr int elem(int T, int j, int n) {
-    if (T == 0) {
-      if (n == cG) return oM;
-      if (n == cFP) return oP;
-      if (n < cDU + D) return oU + (n - cDU);
-      if (DIFF) return (n < cDA + 3) ? oAL + (n - cDA) : ELEM_NONE;
-      if (NT == 1 && n == cDV) return oV + j;
-      return ELEM_NONE;
+  static constexpr int pos(int e) { return grad_pos(D_, VISC, DIFF, e); }
+  /* the 4 operands of a lane -> B operand of tile T, weight j */
+  __device__ static __forceinline__ void pick(const double2 b01, const double2 b23, double (&bop)[NT][NJ]) {
+    const double b[4] = {b01.x, b01.y, b23.x, b23.y};
+    if (NT == 2) {
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) { bop[0][j] = b[0]; bop[NT - 1][j] = b[1 + j]; }
+    } else {
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) bop[0][j] = b[j];
     }
-    if (n == cDV) return oV + j;
-    if (VISC && n >= cFB && n < cFB + D) return oB + j * D + (n - cFB);
-    if (DIFF && n >= cFK && n < cFK + 3) return oK + (n - cFK) * D + j;
-    return ELEM_NONE;
   }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
     /* Eq. 79: grad_i W = (sigma_D / h) f(q) dr_i / r,  f = -3q + 9/4 q^2 (q <= 1), -3/4 (2 - q)^2 (q <= 2) */
@@ -248,37 +301,44 @@ struct GradOp {
     auto S = [&](int T, int j, int c) { return s[(T * NJ + j) * 8 + c]; };
     const double* __restrict__ ra = so.rec_g + i * NREC;
     const double inv = 1.0 / so.sigma_star[i];
-    const double im = 1.0 / ra[oM];
-    const double Pa = ra[oP] * im;
+    const double im = 1.0 / ra[pos(eM)];
+    const double Pa = ra[pos(eP)] * im;
     double G[3] = {0.0, 0.0, 0.0};
     for (int k = 0; k < D; ++k) G[k] = S(0, k, cG);
     double dv = 0.0;
     for (int j = 0; j < D; ++j) dv += S(tDV, j, cDV);
+#pragma unroll
     for (int k = 0; k < 3; ++k) {
       double fp = 0.0, fb = 0.0;
       if (k < D) {
         fp = fma(Pa, G[k], S(0, k, cFP));
         if (VISC) {
           for (int j = 0; j < D; ++j) fb += S(1, j, cFB + k);
-          for (int j = 0; j < D; ++j) fb = fma(ra[oB + j * D + k] * im, G[j], fb);
+#pragma unroll
+          for (int j = 0; j < D; ++j) fb = fma(ra[pos(VISC ? eB + j * D + (k < D ? k : 0) : 0)] * im, G[j], fb);
         }
-        dv = fma(-(ra[oV + k] * im), G[k], dv);
+        dv = fma(-(ra[pos(eV + (k < D ? k : 0))] * im), G[k], dv);
       }
       so.FP[k][i] = fp;
       so.FB[k][i] = fb;
     }
+#pragma unroll
     for (int j = 0; j < 3; ++j)
+#pragma unroll
       for (int k = 0; k < 3; ++k)
-        so.DU[j * 3 + k][i] = (j < D && k < D) ? fma(-(ra[oU + k] * im), G[j], S(0, j, cDU + k)) * inv : 0.0;
+        so.DU[j * 3 + k][i] = (j < D && k < D) ? fma(-(ra[pos(eU + (k < D ? k : 0))] * im), G[j], S(0, j, cDU + k)) * inv : 0.0;
+#pragma unroll
     for (int qq = 0; qq < 3; ++qq) {
       double fk = 0.0;
       if (DIFF) {
         for (int j = 0; j < D; ++j) fk += S(1, j, cFK + qq);
-        for (int j = 0; j < D; ++j) fk = fma(ra[oK + qq * D + j] * im, G[j], fk);
+#pragma unroll
+        for (int j = 0; j < D; ++j) fk = fma(ra[pos(DIFF ? eK + qq * D + j : 0)] * im, G[j], fk);
       }
       so.FK[qq][i] = fk;
+#pragma unroll
       for (int j = 0; j < 3; ++j)
-        so.DA[qq * 3 + j][i] = (DIFF && j < D) ? fma(-(ra[oAL + qq] * im), G[j], S(0, j, cDA + qq)) * inv : 0.0;
+        so.DA[qq * 3 + j][i] = (DIFF && j < D) ? fma(-(ra[pos(DIFF ? eAL + qq : 0)] * im), G[j], S(0, j, cDA + qq)) * inv : 0.0;
     }
     so.divv[i] = dv * inv;
   }
@@ -291,7 +351,7 @@ struct GradOp {
 template <int D_>
 struct EpsGradOp {
   static constexpr int D = D_;
-  static constexpr bool HASH = false, COUNT = false;
+  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = false;
   static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3;
   static constexpr int elem(int, int, int n) { return (n <= 1) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
@@ -539,8 +599,10 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
       }
   }
   __syncthreads();
+  const uint32_t lane_goff = (uint32_t)((GREC_B0 / 2 + 2 * gid) * CSTRIDE) * 16u;   /* GIDMAJOR: byte offset of the lane's operands */
   uint32_t boff[NT][NJ];
   auto load_boff = [&]() {
+    if (Op::GIDMAJOR) return;
 #pragma unroll
     for (int T = 0; T < NT; ++T)
 #pragma unroll
@@ -576,10 +638,15 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
     double aw[NJ], bop[NT][NJ];
     Op::weights(kp, pg, aw);
     const unsigned char* rb = reinterpret_cast<const unsigned char*>(p);
+    if constexpr (Op::GIDMAJOR) {
+      const double2* pl = reinterpret_cast<const double2*>(rb + lane_goff);       /* units 2 + 2 gid and the next one */
+      Op::pick(pl[0], pl[CSTRIDE], bop);
+    } else {
 #pragma unroll
-    for (int T = 0; T < NT; ++T)
+      for (int T = 0; T < NT; ++T)
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) bop[T][j] = *reinterpret_cast<const double*>(rb + boff[T][j]);
+        for (int j = 0; j < NJ; ++j) bop[T][j] = *reinterpret_cast<const double*>(rb + boff[T][j]);
+    }
     if (Op::COUNT) hits[gg] += pg.hit ? 1u : 0u;
     if (Op::HASH) {
       const uint32_t slot = __float_as_uint(payx[koff >> 4].w);  /* sorted slot of the candidate (pack_smoothing_kernel) */

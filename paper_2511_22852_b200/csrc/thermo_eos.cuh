@@ -485,30 +485,45 @@ thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x
   else load_dissip<2>(kp, gm, Y, npad, a, u, ds);
   const double sst2 = sst * sst;
   const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
-  /* AoS payload record of the gradient pass (layout GLayout): x[D], m, then m times each of P, u[D], v[D], B[D*D],
-     K[3*D], alpha[3] — the pair pass multiplies a column of b by the pair weight without m_b (pair_mma.cuh) */
+  /* AoS payload record of the gradient pass (pair_mma.cuh): x, y, z, 0, then the elements m, m P, m u[D], m v[D],
+     m B[D*D], m K[3*D], m alpha[3] stored per MMA column — the pair pass multiplies a column of b by the pair weight
+     without m_b */
   const GLayout L = make_glayout(D, kp.shear != 0, kp.diff != 0);
-  double* __restrict__ rg = so.rec_g + i * L.NREC;
+  double el[32];
+#pragma unroll
+  for (int k = 0; k < 32; ++k) el[k] = 0.0;
   const double mb = Y[CCAKE_MASS * npad + a];
-  for (int k = 0; k < D; ++k) rg[k] = so.x[k][i];
-  rg[L.M] = mb;
-  rg[L.P] = mb * ((th.p + ds.bulkt * sig) / sst2);
-  for (int j = 1; j <= D; ++j) { rg[L.U + j - 1] = mb * u[j]; rg[L.V + j - 1] = mb * (u[j] / gam); }
+  el[L.M] = mb;
+  el[L.P] = mb * ((th.p + ds.bulkt * sig) / sst2);
+  for (int j = 1; j <= D; ++j) { el[L.U + j - 1] = mb * u[j]; el[L.V + j - 1] = mb * (u[j] / gam); }
   if (kp.shear)
     for (int j = 1; j <= D; ++j)
       for (int k = 1; k <= D; ++k) {
         const double pi_j_k = sig * ds.pit[j][k] * glo[k];
         const double pi_0_k = sig * ds.pit[0][k] * glo[k];
-        rg[L.B + (j - 1) * D + (k - 1)] = mb * ((pi_j_k - (u[j] / gam) * pi_0_k) / sst2);
+        el[L.B + (j - 1) * D + (k - 1)] = mb * ((pi_j_k - (u[j] / gam) * pi_0_k) / sst2);
       }
   if (kp.diff) {
     for (int q = 0; q < NQ; ++q) {
-      rg[L.AL + q] = mb * (th.mu[q] / th.T);
+      el[L.AL + q] = mb * (th.mu[q] / th.T);
       for (int j = 1; j <= D; ++j)
-        rg[L.K + q * D + (j - 1)] = mb * ((sig * ds.Jt[q][j] - (u[j] / gam) * sig * ds.Jt[q][0]) / sst2);
+        el[L.K + q * D + (j - 1)] = mb * ((sig * ds.Jt[q][j] - (u[j] / gam) * sig * ds.Jt[q][0]) / sst2);
     }
   }
-  for (int k = L.AL + (kp.diff ? 3 : 0); k < L.NREC; ++k) rg[k] = 0.0;
+  double* __restrict__ rg = so.rec_g + i * GREC_D;
+  reinterpret_cast<double2*>(rg)[0] = make_double2(so.x[0][i], so.x[1][i]);
+  reinterpret_cast<double2*>(rg)[1] = make_double2(so.x[2][i], 0.0);
+  const int variant = (D == 3 ? 4 : 0) + (kp.shear ? 2 : 0) + (kp.diff ? 1 : 0);
+  switch (variant) {
+    case 0: write_grad_record<2, false, false>(rg, el); break;
+    case 1: write_grad_record<2, false, true>(rg, el); break;
+    case 2: write_grad_record<2, true, false>(rg, el); break;
+    case 3: write_grad_record<2, true, true>(rg, el); break;
+    case 4: write_grad_record<3, false, false>(rg, el); break;
+    case 5: write_grad_record<3, false, true>(rg, el); break;
+    case 6: write_grad_record<3, true, false>(rg, el); break;
+    default: write_grad_record<3, true, true>(rg, el); break;
+  }
 }
 
 }  // namespace ccake
