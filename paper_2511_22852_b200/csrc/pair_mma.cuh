@@ -785,10 +785,16 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
         uint32_t nibs = 0u;                                       /* lane q: the 4 union bits of quad q */
         const int nfull = tl >> 2;
         const uint16_t* fq = ff + tig;
+        if (MC == 1) {
 #pragma unroll 1
-        for (int q = 0; q < nfull; ++q) {
-          const uint32_t nib = quad(gg, fq[4 * q], true);
-          if (MC == 1) nibs = (lane == q) ? nib : nibs;
+          for (int q = 0; q < nfull; ++q) {
+            const uint32_t nib = quad(gg, fq[4 * q], true);
+            nibs = (lane == q) ? nib : nibs;
+          }
+        } else {
+          const uint16_t* fend = fq + 4 * nfull;
+#pragma unroll 1
+          for (const uint16_t* fp = fq; fp != fend; fp += 4) quad(gg, *fp, true);
         }
         if (tl & 3) {
           const bool act = 4 * nfull + tig < tl;
