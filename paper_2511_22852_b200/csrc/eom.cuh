@@ -268,11 +268,16 @@ struct RkArgs {
   int update;           /* 0: rates only (refresh)                 */
 };
 
-#ifndef CCAKE_EOM_MINB
-#define CCAKE_EOM_MINB 2
+/* resident blocks per SM the register budget is set for.  3-D (C4): 2 -> 1.57 ms, 3 -> 1.41, 4 -> 1.35, 5 -> 1.64, 6 -> 1.98 per
+   substep; 2-D (C3): 2 -> 0.130 ms, 3 -> 0.111, 4 -> 0.105 */
+#ifndef CCAKE_EOM_MINB3
+#define CCAKE_EOM_MINB3 4
+#endif
+#ifndef CCAKE_EOM_MINB2
+#define CCAKE_EOM_MINB2 4
 #endif
 template <int D, bool DIAG>
-__global__ void __launch_bounds__(128, CCAKE_EOM_MINB)
+__global__ void __launch_bounds__(128, (D == 3) ? CCAKE_EOM_MINB3 : CCAKE_EOM_MINB2)
 eom_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_off, int64_t npad, Sorted so, RkArgs rk,
            uint32_t field_mask, Status* __restrict__ status) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;

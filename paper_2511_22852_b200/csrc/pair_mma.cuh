@@ -602,11 +602,12 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   const uint32_t lane_goff = (uint32_t)((GREC_B0 / 2 + 2 * gid) * CSTRIDE) * 16u;   /* GIDMAJOR: byte offset of the lane's operands */
   uint32_t boff[NT][NJ];
   auto load_boff = [&]() {
-    if (Op::GIDMAJOR) return;
+    if constexpr (!Op::GIDMAJOR) {
 #pragma unroll
-    for (int T = 0; T < NT; ++T)
+      for (int T = 0; T < NT; ++T)
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) boff[T][j] = *reinterpret_cast<volatile uint32_t*>(&s_boff[T * NJ + j][gid]);
+        for (int j = 0; j < NJ; ++j) boff[T][j] = *reinterpret_cast<volatile uint32_t*>(&s_boff[T * NJ + j][gid]);
+    }
   };
   load_boff();
 
