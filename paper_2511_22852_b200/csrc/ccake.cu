@@ -275,8 +275,16 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in)
   if ((rc = mark(c))) return rc;
   /* a5 */
   cudaMemsetAsync(&c->status->n_oob, 0, sizeof(unsigned long long), st);
-  thermo_kernel<<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, c->tb, Ycur, np, c->so, c->status, rk_in.update, c->orig[0],
-                                               rk_in.n_own);
+  {
+    const bool tv = kp.shear != 0, tf = kp.diff != 0;
+#define CCAKE_THERMO_LAUNCH(V, F) thermo_kernel<D, V, F><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, c->tb, Ycur, np, c->so, c->status, \
+                                                                                     rk_in.update, c->orig[0], rk_in.n_own)
+    if (tv && tf) CCAKE_THERMO_LAUNCH(true, true);
+    else if (tv) CCAKE_THERMO_LAUNCH(true, false);
+    else if (tf) CCAKE_THERMO_LAUNCH(false, true);
+    else CCAKE_THERMO_LAUNCH(false, false);
+#undef CCAKE_THERMO_LAUNCH
+  }
   if ((rc = mark(c))) return rc;
   /* a6 */
   launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
