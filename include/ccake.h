@@ -205,7 +205,11 @@ int ccake_slab_info(ccake_ctx* c, int64_t out[4]);
 /* Global ids by load index, n_own + ghosts entries. */
 int ccake_slab_gids(ccake_ctx* c, uint32_t* out, int64_t capacity, int32_t memspace);
 
-/* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load. */
+/* Enqueue nsteps full RK steps (each 2 or 4 substeps a1-a8).  Asynchronous.  ESTATE before a load or on a slab context.
+ * On a stream other than the legacy default stream the launch sequence of a step is captured once as a CUDA graph (the
+ * current time lives in device memory, so the kernel arguments do not change from step to step) and replayed; the results
+ * are bit-identical to launching the kernels one by one (environment CCAKE_NO_GRAPH=1 forces the latter, as does
+ * ccake_enable_timing). */
 int ccake_step(ccake_ctx* c, int32_t nsteps);
 
 /* Wait for the stream.  ERANGE when, since the last load, a particle left the EoS table, a per-particle solve
