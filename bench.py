@@ -317,28 +317,31 @@ def slab_probe(device, steps=5):
     one.close()
     axis, K = 0, 2
     planes = S.slab_planes(w.fields[B.R1 + axis], K)
-    width = S.slab_halo_width(p["h"], p["dx0"])
-    slabs = {}
-    for k in range(K):
-        lo, hi = S.slab_bounds(planes, k)
-        sel = np.nonzero((w.fields[B.R1 + axis] >= lo) & (w.fields[B.R1 + axis] < hi))[0]
-        g = ctx()
-        g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), int(0.9 * w.n), axis, lo, hi, width)
-        slabs[k] = g
-    drv = S.SlabDriver(slabs, K, 2, int(0.5 * w.n), lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev))
-    with torch.cuda.stream(stream):
-        ms_slabs = timed(drv.step)
-        b0 = drv.bytes_moved
-        drv.step(1)
-        per_step = drv.bytes_moved - b0
-        drv.refresh_ghosts()
-    info = [g.slab_info() for g in slabs.values()]
-    for g in slabs.values():
-        g.close()
-    return {"event_particles": w.n, "slabs": K, "axis": "x", "halo_width_fm": width, "ms_per_step_one_context": ms_one,
-            "ms_per_step_slabs_same_gpu": ms_slabs, "owned_per_slab": [i[0] for i in info], "ghosts_per_slab": [i[1] + i[2] for i in info],
-            "message_bytes_per_step": per_step,
-            "note": "2 contexts on one GPU, run one after the other: the cost of the decomposition, not a scaling number"}
+    out = {"event_particles": w.n, "slabs": K, "axis": "x", "ms_per_step_one_context": ms_one,
+           "note": "2 contexts on one GPU, run one after the other: the cost of the decomposition, not a scaling number"}
+    for narrow in (False, True):
+        width = S.slab_halo_width(p["h"], p["dx0"], narrow)
+        slabs = {}
+        for k in range(K):
+            lo, hi = S.slab_bounds(planes, k)
+            sel = np.nonzero((w.fields[B.R1 + axis] >= lo) & (w.fields[B.R1 + axis] < hi))[0]
+            g = ctx()
+            g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), int(0.9 * w.n), axis, lo, hi, width)
+            slabs[k] = g
+        drv = S.SlabDriver(slabs, K, 2, int(0.5 * w.n), lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev), narrow=narrow)
+        with torch.cuda.stream(stream):
+            ms_slabs = timed(drv.step)
+            b0 = drv.bytes_moved
+            drv.step(1)
+            per_step = drv.bytes_moved - b0
+            drv.refresh_ghosts()
+        info = [g.slab_info() for g in slabs.values()]
+        for g in slabs.values():
+            g.close()
+        out["narrow_halo" if narrow else "wide_halo"] = {
+            "halo_width_fm": width, "exchanges_per_substep": 2 if narrow else 1, "ms_per_step_slabs_same_gpu": ms_slabs,
+            "owned_per_slab": [i[0] for i in info], "ghosts_per_slab": [i[1] + i[2] for i in info], "message_bytes_per_step": per_step}
+    return out
 
 
 def run_slabs(args):
@@ -361,7 +364,7 @@ def run_slabs(args):
     K = max(world, 2) if world == 1 else world
     axis = 0
     planes = S.slab_planes(w.fields[B.R1 + axis], K)
-    width = S.slab_halo_width(p["h"], p["dx0"])
+    width = S.slab_halo_width(p["h"], p["dx0"], narrow=True)
     stream = torch.cuda.Stream()
     tab = torch.as_tensor(w.table["data"], device=dev)
     slabs = {}
@@ -372,7 +375,8 @@ def run_slabs(args):
         g.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], tab)
         g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), w.n, axis, lo, hi, width)
         slabs[k] = g
-    drv = S.SlabDriver(slabs, K, 2, w.n // 2, lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev), rank=rank, world=world)
+    drv = S.SlabDriver(slabs, K, 2, w.n // 2, lambda r, c: torch.zeros((r, c), dtype=torch.float64, device=dev), rank=rank, world=world,
+                       narrow=True)
     with torch.cuda.stream(stream):
         drv.step(max(args.warmup, 3))
         torch.cuda.synchronize()
@@ -391,7 +395,7 @@ def run_slabs(args):
         print(json.dumps({"metric": METRIC, "value": w.n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                           "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
                           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                          "config": {"workload": "one C4 event (80 x 80 x 31 = 198,400 particles) cut into %d slabs along x, halo %.2f fm" % (K, width),
+                          "config": {"workload": "one C4 event (80 x 80 x 31 = 198,400 particles) cut into %d slabs along x, halo %.2f fm, gradient records exchanged" % (K, width),
                                      "decomposition": "slabs", "slabs": K}, "gpu_launches": launches}), flush=True)
     for g in slabs.values():
         g.close()

@@ -32,7 +32,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_invert_forward_table", "ccake_smear_sources",
            "ccake_set_sources",
-           "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep",
+           "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep", "ccake_slab_substep_part", "ccake_slab_export_records", "ccake_slab_import_records",
            "ccake_slab_export_migrants", "ccake_slab_import_migrants", "ccake_slab_commit", "ccake_slab_info", "ccake_slab_gids",
            "ccake_step",
            "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
@@ -85,6 +85,9 @@ def lib():
         L.ccake_slab_export_halo.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64)]
         L.ccake_slab_import_ghosts.argtypes = [vp, i32, i32, vp, i64, i64]
         L.ccake_slab_substep.argtypes = [vp, i32]
+        L.ccake_slab_substep_part.argtypes = [vp, i32, i32]
+        L.ccake_slab_export_records.argtypes = [vp, i32, vp, i64, C.POINTER(i64)]
+        L.ccake_slab_import_records.argtypes = [vp, i32, vp, i64, i64]
         L.ccake_slab_export_migrants.argtypes = [vp, i32, vp, i64, C.POINTER(i64)]
         L.ccake_slab_import_migrants.argtypes = [vp, i32, vp, i64, i64]
         L.ccake_slab_commit.argtypes = [vp, C.POINTER(i64)]
@@ -338,6 +341,19 @@ class Ccake:
 
     def slab_substep(self, k):
         self._chk(lib().ccake_slab_substep(self._h, int(k)), "ccake_slab_substep")
+
+    def slab_substep_part(self, k, part):
+        self._chk(lib().ccake_slab_substep_part(self._h, int(k), int(part)), "ccake_slab_substep_part")
+
+    def slab_export_records(self, side, buf):
+        cnt = C.c_int64(0)
+        self._chk(lib().ccake_slab_export_records(self._h, int(side), buf.data_ptr(), int(buf.shape[1]), C.byref(cnt)),
+                  "ccake_slab_export_records")
+        return int(cnt.value)
+
+    def slab_import_records(self, side, buf, count):
+        self._chk(lib().ccake_slab_import_records(self._h, int(side), buf.data_ptr() if buf is not None else None,
+                                                  int(buf.shape[1]) if buf is not None else 0, int(count)), "ccake_slab_import_records")
 
     def slab_export_migrants(self, side, buf):
         cnt = C.c_int64(0)

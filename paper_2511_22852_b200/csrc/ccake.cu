@@ -96,6 +96,7 @@ struct ccake_ctx {
   bool inv_valid = false;           /* slot_of[] matches the current store order */
   uint32_t *gid = nullptr, *gid_new = nullptr;   /* global particle id by load index */
   uint32_t *slot_of = nullptr;      /* store slot of a load index (inverse of orig) */
+  uint32_t *sorted_of = nullptr;    /* sorted slot of a store slot (inverse of perm), for the record exchange */
   uint32_t *sflag[3] = {nullptr, nullptr, nullptr}, *stot[3] = {nullptr, nullptr, nullptr};   /* selection flags / ranks, chunk totals */
   uint32_t *halo_list[2] = {nullptr, nullptr};   /* load indices exported to each side in this step */
   int64_t mig_in[2] = {0, 0};       /* migrants received from each side, parked behind the ghosts until the commit */
@@ -146,6 +147,7 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->src); c->src = nullptr; c->has_src = false;
   cudaFree(c->gid); c->gid = nullptr; cudaFree(c->gid_new); c->gid_new = nullptr;
   cudaFree(c->slot_of); c->slot_of = nullptr;
+  cudaFree(c->sorted_of); c->sorted_of = nullptr;
   for (int k = 0; k < 3; ++k) { cudaFree(c->sflag[k]); c->sflag[k] = nullptr; cudaFree(c->stot[k]); c->stot[k] = nullptr; }
   for (int k = 0; k < 2; ++k) { cudaFree(c->halo_list[k]); c->halo_list[k] = nullptr; }
   cudaFree(c->mig_buf); c->mig_buf = nullptr;
@@ -258,12 +260,15 @@ void drop_graphs(ccake_ctx* c) {
   c->graphs.clear();
 }
 
+/* parts: 1 = pack, candidate lists, a4, a5;  2 = a6, a7 + a8;  3 = the whole rest of the substep.  (The slab decomposition
+   with narrow halos exchanges the gradient records of the halo particles between the two parts.) */
 template <int D>
-int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in) {
+int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in, int parts = 3) {
   const int64_t N = c->N, np = c->npad;
   cudaStream_t st = c->stream;
   const KParams& kp = c->kp;
   int rc;
+  if (parts & 1) {
   pack_smoothing_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->so.perm, c->grid, c->so);
   if ((rc = mark(c))) return rc;
   /* a4 */
@@ -286,6 +291,9 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in)
 #undef CCAKE_THERMO_LAUNCH
   }
   if ((rc = mark(c))) return rc;
+  c->launches += 3;
+  }
+  if (!(parts & 2)) return launch_check(c, "substep (part 1)");
   /* a6 */
   launch_gradient<D>(N, kp, c->grid, c->so, kp.shear != 0, kp.diff != 0, st);
   if ((rc = mark(c))) return rc;
@@ -298,25 +306,27 @@ int pair_and_eom(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk_in)
   if (rk.diag) eom_kernel<D, true><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, np, c->so, rk, c->field_mask, c->status);
   else eom_kernel<D, false><<<nblk(N, 128), 128, 0, st>>>(N, kp, c->x0_dev, x0_off, np, c->so, rk, c->field_mask, c->status);
   if ((rc = mark(c))) return rc;
-  c->launches += 5;
+  c->launches += 2;
   return launch_check(c, "substep");
 }
 
-int substep(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk) {
+int substep(ccake_ctx* c, double* Ycur, double x0_off, const RkArgs& rk, int parts = 3) {
   int rc;
-  if ((rc = mark(c))) return rc;
-  if ((rc = build_cells(c, Ycur, false))) return rc;
-  if ((rc = mark(c))) return rc;
-  if (c->P.dim == 2) rc = pair_and_eom<2>(c, Ycur, x0_off, rk);
-  else rc = pair_and_eom<3>(c, Ycur, x0_off, rk);
-  if (c->timing) c->substeps_timed++;
+  if (parts & 1) {
+    if ((rc = mark(c))) return rc;
+    if ((rc = build_cells(c, Ycur, false))) return rc;
+    if ((rc = mark(c))) return rc;
+  }
+  if (c->P.dim == 2) rc = pair_and_eom<2>(c, Ycur, x0_off, rk, parts);
+  else rc = pair_and_eom<3>(c, Ycur, x0_off, rk, parts);
+  if (c->timing && (parts & 2)) c->substeps_timed++;
   return rc;
 }
 
 /* substep k of the RK scheme (DESIGN reading 7).  RK2 midpoint: k1 = f(y0, x0); yh = y0 + dt/2 k1; k2 = f(yh, x0 + dt/2);
    y1 = y0 + dt k2.  Classical RK4 with the accumulator Y[2].  Substep 0 reorders Y[0] into Y[1] and swaps, so "base" and
    "out" are named after the swap; the last substep advances the time. */
-int rk_substep(ccake_ctx* c, int k) {
+int rk_substep(ccake_ctx* c, int k, int parts = 3) {
   const double dt = c->P.dx0;
   const bool rk2 = c->P.integrator == 2;
   const int nsub = rk2 ? 2 : 4;
@@ -328,14 +338,16 @@ int rk_substep(ccake_ctx* c, int k) {
   double off = 0.0;
   if (k == 0) {
     double* Ycur = c->Y[0];
-    if ((rc = mark(c))) return rc;
-    if ((rc = build_cells(c, Ycur, true))) return rc;
-    if ((rc = mark(c))) return rc;
+    if (parts & 1) {
+      if ((rc = mark(c))) return rc;
+      if ((rc = build_cells(c, Ycur, true))) return rc;
+      if ((rc = mark(c))) return rc;
+    }
     rk.Ybase = c->Y[0]; rk.Yout = c->Y[1]; rk.c_out = 0.5 * dt;
     if (!rk2) { rk.Yacc = c->Y[2]; rk.acc_mode = 1; rk.w_acc = 1.0; }
-    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk) : pair_and_eom<3>(c, Ycur, 0.0, rk);
+    rc = (c->P.dim == 2) ? pair_and_eom<2>(c, Ycur, 0.0, rk, parts) : pair_and_eom<3>(c, Ycur, 0.0, rk, parts);
     if (rc) return rc;
-    if (c->timing) c->substeps_timed++;
+    if (c->timing && (parts & 2)) c->substeps_timed++;
   } else {
     rk.Ybase = c->Y[0];
     if (rk2) { rk.Yout = c->Y[0]; rk.c_out = dt; off = 0.5 * dt; }
@@ -345,9 +357,9 @@ int rk_substep(ccake_ctx* c, int k) {
       else if (k == 2) { rk.Yout = c->Y[1]; rk.c_out = dt; rk.acc_mode = 2; rk.w_acc = 2.0; off = 0.5 * dt; }
       else { rk.Yout = c->Y[0]; rk.c_out = dt / 6.0; rk.acc_mode = 3; rk.w_acc = 2.0; off = dt; }
     }
-    if ((rc = substep(c, c->Y[1], off, rk))) return rc;
+    if ((rc = substep(c, c->Y[1], off, rk, parts))) return rc;
   }
-  if (k == nsub - 1) {
+  if (k == nsub - 1 && (parts & 2)) {
     advance_time_kernel<<<1, 1, 0, c->stream>>>(c->x0_dev, dt);    /* x0 <- x0 + dt, the same operation as on the host below */
     c->launches += 1;
     c->x0 = c->x0 + dt;
@@ -1106,6 +1118,7 @@ int slab_alloc(ccake_ctx* c) {
   CK(cudaMalloc(&c->gid, sizeof(uint32_t) * cap));
   CK(cudaMalloc(&c->gid_new, sizeof(uint32_t) * cap));
   CK(cudaMalloc(&c->slot_of, sizeof(uint32_t) * cap));
+  CK(cudaMalloc(&c->sorted_of, sizeof(uint32_t) * cap));
   for (int k = 0; k < 3; ++k) {
     CK(cudaMalloc(&c->sflag[k], sizeof(uint32_t) * cap));
     CK(cudaMalloc(&c->stot[k], sizeof(uint32_t) * nch));
@@ -1254,6 +1267,52 @@ int ccake_slab_substep(ccake_ctx* c, int32_t k) {
   rc = rk_substep(c, k);
   if (k == 0) c->inv_valid = false;            /* the store was reordered */
   return rc;
+}
+
+int ccake_slab_substep_part(ccake_ctx* c, int32_t k, int32_t part) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_substep_part");
+  if (rc) return rc;
+  const int nsub = (c->P.integrator == 2) ? 2 : 4;
+  if (k < 0 || k >= nsub || (part != 1 && part != 2)) { c->err = "substep index or part out of range"; return CCAKE_EINVAL; }
+  if (c->P.eos_kind == 1 && !c->table_loaded) { c->err = "step before table load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  rc = rk_substep(c, k, part);
+  if (k == 0 && part == 1) c->inv_valid = false;            /* the store was reordered */
+  return rc;
+}
+
+int ccake_slab_export_records(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_export_records");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || !buf || buf_cap <= 0 || !count) { c->err = "bad arguments to ccake_slab_export_records"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  const int64_t cnt = c->halo_cnt[side];
+  *count = cnt;
+  if (cnt > buf_cap) { c->err = "record message larger than the buffer"; return CCAKE_ENOMEM; }
+  slab_inverse(c);
+  slab_inverse_perm_kernel<<<nblk(c->N, 256), 256, 0, c->stream>>>(c->so.perm, c->N, c->sorted_of);
+  if (cnt > 0)
+    slab_pack_records_kernel<<<nblk(cnt, 256), 256, 0, c->stream>>>(c->so.rec_g, GREC_D, cnt, c->halo_list[side], c->slot_of, c->sorted_of, buf, buf_cap);
+  c->launches += 2;
+  return launch_check(c, "slab_export_records");
+}
+
+int ccake_slab_import_records(ccake_ctx* c, int32_t side, const double* buf, int64_t buf_cap, int64_t count) {
+  if (!c) return CCAKE_EINVAL;
+  int rc = slab_need(c, "ccake_slab_import_records");
+  if (rc) return rc;
+  if ((side != 0 && side != 1) || count < 0 || (count > 0 && !buf) || buf_cap < count) { c->err = "bad arguments to ccake_slab_import_records"; return CCAKE_EINVAL; }
+  if (count != c->n_ghost[side]) { c->err = "record message differs in size from the ghosts of that side"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  slab_inverse(c);
+  slab_inverse_perm_kernel<<<nblk(c->N, 256), 256, 0, c->stream>>>(c->so.perm, c->N, c->sorted_of);
+  const int64_t load0 = c->n_own + (side == 0 ? 0 : c->n_ghost[0]);
+  if (count > 0)
+    slab_unpack_records_kernel<<<nblk(count, 256), 256, 0, c->stream>>>(c->so.rec_g, GREC_D, load0, count, buf, buf_cap, c->slot_of, c->sorted_of);
+  c->launches += 2;
+  return launch_check(c, "slab_import_records");
 }
 
 int ccake_slab_export_migrants(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count) {

@@ -12,6 +12,10 @@
  *   step:  export_halo(k = 0) -> import_ghosts(k = 0) -> substep 0 -> [ export_halo(k) -> import_ghosts(k) -> substep k ] ...
  *          -> export_migrants -> import_migrants -> commit (owned set rebuilt: stayers in store order, then arrivals)
  *
+ * With NARROW halos (W = 2h + drift) the ghosts' own sums are incomplete; then the gradient records of the halo particles
+ * travel as a second message between a5 and a6 (substep_a -> export_records -> import_records -> substep_b): half the ghosts,
+ * twice the messages.
+ *
  * Exchange buffers (device memory of the caller, moved by the caller's transport: a device copy, or NCCL send/recv):
  * SLAB_NF rows of `cap` doubles, row f < NSTATE = state field f, row NSTATE = the global particle id; entry i of
  * every row belongs to particle i of the message.  Selection is by flags + exclusive scan (grid_sort.cuh), so the order
@@ -144,6 +148,32 @@ __global__ void slab_park_kernel(const double* __restrict__ in, int64_t cap_in, 
   if (i >= cnt) return;
 #pragma unroll 4
   for (int f = 0; f < SLAB_NF; ++f) park[(int64_t)f * cap + col0 + i] = in[(int64_t)f * cap_in + i];
+}
+
+/* ---- narrow halos: the gradient records of the halo particles travel between a5 and a6 ---- */
+/* sorted slot of a store slot (inverse of perm) */
+__global__ void slab_inverse_perm_kernel(const uint32_t* __restrict__ perm, int64_t n, uint32_t* __restrict__ sorted_of) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) sorted_of[perm[i]] = (uint32_t)i;
+}
+
+/* message: nrec rows of cap doubles, entry i = the record of load index list[i] (the halo list of this step) */
+__global__ void slab_pack_records_kernel(const double* __restrict__ rec, int nrec, int64_t cnt, const uint32_t* __restrict__ list,
+                                         const uint32_t* __restrict__ slot_of, const uint32_t* __restrict__ sorted_of,
+                                         double* __restrict__ buf, int64_t cap) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= cnt) return;
+  const double* __restrict__ r = rec + (int64_t)sorted_of[slot_of[list[i]]] * nrec;
+  for (int f = 0; f < nrec; ++f) buf[(int64_t)f * cap + i] = r[f];
+}
+
+/* the records of the ghosts with load indices load0 + i are overwritten with their owners' */
+__global__ void slab_unpack_records_kernel(double* __restrict__ rec, int nrec, int64_t load0, int64_t cnt, const double* __restrict__ buf,
+                                           int64_t cap, const uint32_t* __restrict__ slot_of, const uint32_t* __restrict__ sorted_of) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= cnt) return;
+  double* __restrict__ r = rec + (int64_t)sorted_of[slot_of[load0 + i]] * nrec;
+  for (int f = 0; f < nrec; ++f) r[f] = buf[(int64_t)f * cap + i];
 }
 
 __global__ void slab_iota_gid_kernel(uint32_t* __restrict__ gid, int64_t n, uint32_t base) {

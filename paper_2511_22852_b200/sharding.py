@@ -54,6 +54,7 @@ def reduce_totals(totals, device="cpu") -> np.ndarray:
 # the plan (where to cut), the order of the calls, and moving the message buffers: a hand-over inside one process, or
 # torch.distributed send / recv (NCCL between GPUs, gloo in the CPU tests).
 SLAB_ROWS = 29          # 28 state fields + the global particle id
+SLAB_REC_ROWS = 36      # a gradient record (narrow halos): position + the payload columns of the gradient pass
 INF = 1.0e300
 
 
@@ -84,10 +85,11 @@ def slab_bounds(planes, k: int):
     return lo, hi
 
 
-def slab_halo_width(h: float, dx0: float) -> float:
-    """Two kernel supports (smoothing sums of the neighbours of an owned particle are recomputed on ghosts) plus the drift
-    of the particles on both sides during one step (|v| < 1)."""
-    return 4.0 * h + 2.0 * dx0
+def slab_halo_width(h: float, dx0: float, narrow: bool = False) -> float:
+    """Wide halos: two kernel supports (the smoothing sums of the neighbours of an owned particle are recomputed on ghosts)
+    plus the drift of the particles on both sides during one step (|v| < 1).  Narrow halos: one kernel support plus the
+    drift; the gradient records of the ghosts then come from their owners in a second message per substep."""
+    return (2.0 if narrow else 4.0) * h + 2.0 * dx0
 
 
 def slab_owner(k: int, n_slabs: int, world: int) -> int:
@@ -104,21 +106,25 @@ class SlabDriver:
     tensor on the right device).  Neighbouring slabs on the same rank hand their messages over directly; slabs on other
     ranks are reached with torch.distributed point-to-point calls, all messages of a phase posted together."""
 
-    def __init__(self, local: dict, n_slabs: int, nsub: int, buf_cap: int, new_buffer, rank: int = 0, world: int = 1):
+    def __init__(self, local: dict, n_slabs: int, nsub: int, buf_cap: int, new_buffer, rank: int = 0, world: int = 1,
+                 narrow: bool = False):
         self.local, self.K, self.nsub, self.cap = dict(local), int(n_slabs), int(nsub), int(buf_cap)
         self.rank, self.world = rank, world
         self.new_buffer = new_buffer
-        self.send = {k: [new_buffer(SLAB_ROWS, buf_cap), new_buffer(SLAB_ROWS, buf_cap)] for k in self.local}
-        self.recv = {k: [new_buffer(SLAB_ROWS, buf_cap), new_buffer(SLAB_ROWS, buf_cap)] for k in self.local}
+        self.narrow = bool(narrow)          # the contexts were loaded with slab_halo_width(..., narrow=True)
+        self.rows = SLAB_REC_ROWS if narrow else SLAB_ROWS        # one buffer size serves both kinds of message
+        self.send = {k: [new_buffer(self.rows, buf_cap), new_buffer(self.rows, buf_cap)] for k in self.local}
+        self.recv = {k: [new_buffer(self.rows, buf_cap), new_buffer(self.rows, buf_cap)] for k in self.local}
         self.bytes_moved = 0
 
     def _neighbour(self, k, side):
         nb = k - 1 if side == 0 else k + 1
         return nb if 0 <= nb < self.K else None
 
-    def _exchange(self, export, accept):
+    def _exchange(self, export, accept, rows=SLAB_ROWS):
         """One phase: every local slab exports towards both faces, the messages travel, every local slab accepts what
-        arrived at its faces (low face first).  export(k, side, buf) -> count; accept(k, side, buf, count)."""
+        arrived at its faces (low face first).  export(k, side, buf) -> count; accept(k, side, buf, count).  rows = rows of
+        a message that carry data (the buffers may have more)."""
         import torch
         arrived = {}                      # (slab, side) -> (buffer, count)
         remote = []                       # (dst rank, dst slab, dst side, buffer, count)
@@ -130,7 +136,7 @@ class SlabDriver:
                 cnt = export(k, side, self.send[k][side])
                 if cnt > self.cap:
                     raise RuntimeError("slab message exceeds the buffer capacity")
-                self.bytes_moved += 8 * SLAB_ROWS * cnt
+                self.bytes_moved += 8 * rows * cnt
                 if nb in self.local:
                     arrived[(nb, 1 - side)] = (self.send[k][side], cnt)
                 else:
@@ -149,8 +155,8 @@ class SlabDriver:
                 for w in dist.batch_isend_irecv(ops):
                     w.wait()
             counts = [int(t.item()) for t in rcnt]
-            sdat = [b[:, :c].contiguous() for (_, _, _, b, c) in remote]
-            rdat = [self.new_buffer(SLAB_ROWS, max(c, 1))[:, :c].contiguous() for c in counts]
+            sdat = [b[:rows, :c].contiguous() for (_, _, _, b, c) in remote]
+            rdat = [self.new_buffer(rows, max(c, 1))[:, :c].contiguous() for c in counts]
             ops = [dist.P2POp(dist.isend, t, r[0], tag=2 * r[1] + r[2]) for t, r in zip(sdat, remote) if t.numel()]
             ops += [dist.P2POp(dist.irecv, t, e[0], tag=2 * e[1] + e[2]) for t, e in zip(rdat, expect) if t.numel()]
             if ops:
@@ -159,7 +165,7 @@ class SlabDriver:
             for (src, k, side), t, c in zip(expect, rdat, counts):
                 if c > self.cap:
                     raise RuntimeError("slab message exceeds the buffer capacity")
-                self.recv[k][side][:, :c] = t
+                self.recv[k][side][:rows, :c] = t
                 arrived[(k, side)] = (self.recv[k][side], c)
         elif remote:
             raise RuntimeError("a neighbouring slab is not local and there is no process group")
@@ -189,8 +195,16 @@ class SlabDriver:
             for s in range(self.nsub):
                 self._exchange(lambda k, side, buf: self.local[k].slab_export_halo(side, s, buf),
                                lambda k, side, buf, cnt: self.local[k].slab_import_ghosts(side, s, buf, cnt))
-                for k in sorted(self.local):
-                    self.local[k].slab_substep(s)
+                if self.narrow:
+                    for k in sorted(self.local):
+                        self.local[k].slab_substep_part(s, 1)                      # a1-a5
+                    self._exchange(lambda k, side, buf: self.local[k].slab_export_records(side, buf),
+                                   lambda k, side, buf, cnt: self.local[k].slab_import_records(side, buf, cnt), rows=SLAB_REC_ROWS)
+                    for k in sorted(self.local):
+                        self.local[k].slab_substep_part(s, 2)                      # a6-a8
+                else:
+                    for k in sorted(self.local):
+                        self.local[k].slab_substep(s)
             self._exchange(lambda k, side, buf: self.local[k].slab_export_migrants(side, buf),
                            lambda k, side, buf, cnt: self.local[k].slab_import_migrants(side, buf, cnt))
             for k in sorted(self.local):
