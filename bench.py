@@ -616,6 +616,7 @@ def run_ours(args):
             "config": {"workload": workload_text(args.config), "particles_per_gpu": w.n, "rk_substeps_per_step": nsub,
                        "ordered_pairs_per_pass": npairs, "l2": "inputs larger than L2 (state + work arrays > 1 GB per substep)"},
             "pair_interactions_per_s": npairs * 2 * nsub * args.steps * world / (ms_total * 1e-3),
+            "pair_interactions_unit": "ordered neighbour pairs (a, b), a != b, r_ab < 2h, per pair pass; 2 passes (a4, a6) per substep",
             "substep_hbm_frac": total_bytes * nsub / (ms_total / args.steps * 1e-3) / 1e9 / hbm,
             "roofline": {"bound": "alu", "kernel": {"grad": "gradient pass a6", "smooth": "smoothing pass a4"}[dom],
                          "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,

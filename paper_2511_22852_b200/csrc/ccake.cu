@@ -1235,10 +1235,10 @@ int ccake_slab_import_ghosts(ccake_ctx* c, int32_t side, int32_t k, const double
   cudaStream_t st = c->stream;
   const int64_t np = c->npad;
   if (k == 0) {
-    if (c->N + count > c->cap) { c->err = "ghosts exceed the capacity of the slab context"; return CCAKE_ENOMEM; }
     /* the low side's ghosts take the load indices right behind the owned particles, the high side's follow */
     if (side == 0 && c->n_ghost[1] > 0) { c->err = "import the low side's ghosts before the high side's"; return CCAKE_ESTATE; }
     if (c->n_ghost[side] > 0) { c->err = "the ghosts of an earlier exchange are still there: ccake_slab_commit first"; return CCAKE_ESTATE; }
+    if (c->N + count > c->cap) { c->err = "ghosts exceed the capacity of the slab context"; return CCAKE_ENOMEM; }
     const int64_t load0 = c->n_own + (side == 0 ? 0 : c->n_ghost[0]);
     if (count > 0)
       slab_append_kernel<<<nblk(count, 256), 256, 0, st>>>(c->Y[0], np, c->N, load0, count, buf, buf_cap, c->orig[0], c->gid);

@@ -190,3 +190,48 @@ def test_slab_calls_are_refused_on_plain_contexts_and_steps_on_slab_contexts():
     for f in (B.S, B.U1):
         assert np.max(np.abs(a[f] - b[f][gid])) <= 1e-12 * max(np.max(np.abs(b[f])), 1e-300)
     g.close(); ref.close()
+
+
+def test_slab_error_paths():
+    """Message larger than the caller's buffer, ghosts beyond the capacity, imports in the wrong order, a second import without
+    a commit: refused with the documented codes, and the context stays usable."""
+    w = _with_flow(W.config_c4(K=1, n_side=12, n_eta=31, nsteps=2, n_hot=4, table=_table()), 9)
+    slabs, drv, planes = _make_slabs(w, 2, 2)
+    lo, hi = slabs[0], slabs[1]
+    small = torch.zeros((S.SLAB_ROWS, 8), dtype=torch.float64, device="cuda:0")
+    big = torch.zeros((S.SLAB_ROWS, w.n), dtype=torch.float64, device="cuda:0")
+    with pytest.raises(B.CcakeError) as e:
+        lo.slab_export_halo(1, 0, small)                      # hundreds of halo particles do not fit 8 columns
+    assert e.value.rc == B.ENOMEM
+    cnt = lo.slab_export_halo(1, 0, big)
+    assert cnt > 8
+    with pytest.raises(B.CcakeError) as e:
+        lo.slab_export_halo(2, 0, big)                        # no such face
+    assert e.value.rc == B.EINVAL
+    hi.slab_import_ghosts(1, 0, big, cnt)                     # (the same particles, standing in for a high neighbour's message)
+    with pytest.raises(B.CcakeError) as e:
+        hi.slab_import_ghosts(0, 0, big, cnt)                 # low side after the high side
+    assert e.value.rc == B.ESTATE
+    hi.slab_commit()
+    hi.slab_import_ghosts(0, 0, big, cnt)
+    with pytest.raises(B.CcakeError) as e:
+        hi.slab_import_ghosts(0, 0, big, cnt)                 # the ghosts of the first import are still there
+    assert e.value.rc == B.ESTATE
+    with pytest.raises(B.CcakeError) as e:
+        hi.slab_import_ghosts(0, 1, big, cnt - 1)             # a later substep must bring the same particles
+    assert e.value.rc == B.EINVAL
+    hi.slab_commit()
+    # a context loaded with no room for ghosts
+    sel = np.nonzero(w.fields[B.R3] >= planes[0])[0]
+    g = B.Ccake(**w.params)
+    g.load_eos_table(w.table["axes"], w.table["axis_kind"], w.table["col_ids"], w.table["data"])
+    g.slab_load({f: np.ascontiguousarray(v[sel]) for f, v in w.fields.items()}, sel.astype(np.uint32), sel.size, 2, planes[0], S.INF, 1.3)
+    with pytest.raises(B.CcakeError) as e:
+        g.slab_import_ghosts(0, 0, big, cnt)
+    assert e.value.rc == B.ENOMEM
+    g.close()
+    # the pair of slabs still runs a step after all that
+    drv.step(1)
+    for s_ in slabs.values():
+        assert s_.conserved_totals()[13] == 0.0
+        s_.close()
