@@ -196,10 +196,10 @@ int ccake_slab_import_ghosts(ccake_ctx* c, int32_t side, int32_t k, const double
 /* Substep k (0 .. 1 for RK2, 0 .. 3 for RK4) of one RK step over owned particles and ghosts; the last one advances the time. */
 int ccake_slab_substep(ccake_ctx* c, int32_t k);
 /* NARROW halos (halo_width >= 2h + 2 dx0 only): the ghosts' own smoothing sums are incomplete, so their gradient records
- * (36 doubles each: position + the payload columns of a6) come from their owners between a5 and a6:
+ * (32 doubles each: the payload columns of a6 and the position) come from their owners between a5 and a6:
  *   ccake_slab_substep_part(k, 1)  [a1-a5]  ->  export_records -> [transport] -> neighbour.import_records  ->
  *   ccake_slab_substep_part(k, 2)  [a6-a8]
- * Record messages have 36 rows of buf_cap doubles, entry i = the i-th particle of this step's halo message of that side. */
+ * Record messages have 32 rows of buf_cap doubles, entry i = the i-th particle of this step's halo message of that side. */
 int ccake_slab_substep_part(ccake_ctx* c, int32_t k, int32_t part);
 int ccake_slab_export_records(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count);
 int ccake_slab_import_records(ccake_ctx* c, int32_t side, const double* buf, int64_t buf_cap, int64_t count);

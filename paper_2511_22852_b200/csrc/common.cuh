@@ -115,7 +115,7 @@ struct Sorted {
   /* a5 */
   double *gamma, *sigma, *s, *n[NQ];
   double *T, *mu[NQ], *p, *e, *cs2, *ws, *wq[NQ];
-  double* rec_g;      /* [n][36]: AoS payload of the gradient pass: x, y, z, 0, then 8 blocks of 4 MMA operands (pair_mma.cuh) */
+  double* rec_g;      /* [n][32]: AoS payload of the gradient pass: 8 blocks of 4 MMA operands, position in the 3 free slots (pair_mma.cuh) */
   /* a6 */
   double *FP[3], *FB[3], *FK[NQ], *DU[9], *DA[9], *divv;
   /* hit masks of the smoothing pass, reused by the gradient pass of the same substep (pair_mma.cuh):

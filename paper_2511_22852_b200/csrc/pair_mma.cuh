@@ -170,7 +170,7 @@ struct SmoothOp {
   static constexpr int D = D_;
   static constexpr bool HASH = HASH_;
   static constexpr bool COUNT = true, GIDMAJOR = false;
-  static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3;
+  static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3, XO = 0;
   static constexpr int elem(int, int, int n) { return (n <= 4) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
     const double q = g.q;
@@ -225,11 +225,13 @@ __host__ __device__ constexpr int grad_elem(int D, bool visc, bool diff, int T, 
   if (diff && n >= cFK && n < cFK + 3) return L.K + (n - cFK) * D + j;
   return ELEM_NONE;
 }
-/* Record (36 doubles): x, y, z, 0, then 8 blocks of 4 doubles, block n = the operands of MMA column n ("gid-major": the 4
+/* Record (32 doubles = 256 bytes): 8 blocks of 4 doubles, block n = the operands of MMA column n ("gid-major": the 4
    operands of lane (gid, tig) are 32 contiguous bytes, two 16-byte loads from one address): slot 0 = column n of tile 0,
    slots 1..3 = column n of tile 1 for j = 0, 1, 2 (viscous / diffusive), or slots 0..2 = column n of the single tile for
-   j = 0, 1, 2 (ideal fluid: only its v_j column depends on j). */
-constexpr int GREC_D = 36, GREC_B0 = 4;
+   j = 0, 1, 2 (ideal fluid: only its v_j column depends on j).  Slots 1..3 of block 7 are free in every variant (tile 1
+   has at most 7 columns, the single tile of the ideal fluid at most 6) and hold the position x, y, z: the MMA column they
+   feed is never read. */
+constexpr int GREC_D = 32, GREC_B0 = 0, GREC_X = 29;
 __host__ __device__ constexpr int grad_slot_elem(int D, bool visc, bool diff, int n, int s) {
   const bool two = visc || diff;
   const int T = two ? (s == 0 ? 0 : 1) : 0;
@@ -267,7 +269,7 @@ struct GradOp {
   static constexpr int eM = make_glayout(D_, VISC, DIFF).M, eP = make_glayout(D_, VISC, DIFF).P, eU = make_glayout(D_, VISC, DIFF).U,
                        eV = make_glayout(D_, VISC, DIFF).V, eB = make_glayout(D_, VISC, DIFF).B, eK = make_glayout(D_, VISC, DIFF).K,
                        eAL = make_glayout(D_, VISC, DIFF).AL;
-  static constexpr int NREC = GREC_D;
+  static constexpr int NREC = GREC_D, XO = GREC_X;
   static constexpr int NJ = D, NT = (VISC || DIFF) ? 2 : 1;
   static constexpr int elem(int, int, int) { return ELEM_NONE; }       /* not used: the operands are found by position */
   /* column positions */
@@ -352,7 +354,7 @@ template <int D_>
 struct EpsGradOp {
   static constexpr int D = D_;
   static constexpr bool HASH = false, COUNT = false, GIDMAJOR = false;
-  static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3;
+  static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3, XO = 0;
   static constexpr int elem(int, int, int n) { return (n <= 1) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
     const double t = 2.0 - g.q;
@@ -549,7 +551,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
       const int64_t ic = (ih[g] < n) ? ih[g] : n - 1;
       xa[g][0] = xa[g][1] = xa[g][2] = 0.0;
 #pragma unroll
-      for (int k = 0; k < D; ++k) xa[g][k] = rec[ic * Op::NREC + k];
+      for (int k = 0; k < D; ++k) xa[g][k] = rec[ic * Op::NREC + Op::XO + k];
       const float4 fa = xf[ic];
       float glo[3] = {fa.x, fa.y, (D == 3) ? fa.z : 0.f}, ghi[3] = {fa.x, fa.y, (D == 3) ? fa.z : 0.f};
 #pragma unroll
@@ -632,10 +634,18 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
      (smoothing pass) the 4 bits "candidate t of the quad is within 2h of at least one home of the group". */
   auto quad = [&](const int gg, const uint32_t koff, const bool act) -> uint32_t {
     const double2* __restrict__ p = reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(pay) + koff);
-    const double2 h0 = p[0];
-    const double zb = (D == 3) ? reinterpret_cast<const double*>(p + CSTRIDE)[0] : 0.0;
+    double xb, yb, zb;
+    if constexpr (Op::GIDMAJOR) {                       /* x in the upper half of unit 14, (y, z) = unit 15 */
+      xb = reinterpret_cast<const double*>(p + (GREC_X / 2) * CSTRIDE)[1];
+      const double2 yz = p[(GREC_X / 2 + 1) * CSTRIDE];
+      yb = yz.x; zb = (D == 3) ? yz.y : 0.0;
+    } else {
+      const double2 h0 = p[0];
+      xb = h0.x; yb = h0.y;
+      zb = (D == 3) ? reinterpret_cast<const double*>(p + CSTRIDE)[0] : 0.0;
+    }
     PairGeom<D> pg;
-    pg.set(kp, xa[gg], h0.x, h0.y, zb, act);
+    pg.set(kp, xa[gg], xb, yb, zb, act);
     double aw[NJ], bop[NT][NJ];
     Op::weights(kp, pg, aw);
     const unsigned char* rb = reinterpret_cast<const unsigned char*>(p);

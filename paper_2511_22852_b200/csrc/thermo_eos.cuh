@@ -491,7 +491,7 @@ thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x
   load_dissip<D>(kp, gm, Y, npad, a, u, ds);
   const double sst2 = sst * sst;
   const double glo[4] = {1.0, -1.0, -1.0, -gm.G3};
-  /* AoS payload record of the gradient pass (pair_mma.cuh): x, y, z, 0, then the elements m, m P, m u[D], m v[D],
+  /* AoS payload record of the gradient pass (pair_mma.cuh): the elements m, m P, m u[D], m v[D],
      m B[D*D], m K[3*D], m alpha[3] stored per MMA column — the pair pass multiplies a column of b by the pair weight
      without m_b */
   constexpr GLayout L = make_glayout(TD, TV, TF);
@@ -522,9 +522,8 @@ thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x
     }
   }
   double* __restrict__ rg = so.rec_g + i * GREC_D;
-  reinterpret_cast<double2*>(rg)[0] = make_double2(so.x[0][i], so.x[1][i]);
-  reinterpret_cast<double2*>(rg)[1] = make_double2(so.x[2][i], 0.0);
   write_grad_record<TD, TV, TF>(rg, el);
+  rg[GREC_X] = so.x[0][i]; rg[GREC_X + 1] = so.x[1][i]; rg[GREC_X + 2] = so.x[2][i];      /* the free slots of block 7 */
 }
 
 }  // namespace ccake

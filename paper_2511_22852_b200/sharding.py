@@ -54,7 +54,7 @@ def reduce_totals(totals, device="cpu") -> np.ndarray:
 # the plan (where to cut), the order of the calls, and moving the message buffers: a hand-over inside one process, or
 # torch.distributed send / recv (NCCL between GPUs, gloo in the CPU tests).
 SLAB_ROWS = 29          # 28 state fields + the global particle id
-SLAB_REC_ROWS = 36      # a gradient record (narrow halos): position + the payload columns of the gradient pass
+SLAB_REC_ROWS = 32      # a gradient record (narrow halos): the payload columns of the gradient pass and the position
 INF = 1.0e300
 
 
