@@ -228,6 +228,13 @@ int ccake_synchronize(ccake_ctx* c);
 int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* field_ids, double* const* cols,
                       int64_t capacity, int32_t memspace);
 
+/* The same into HOST buffers without waiting for them: the fields are gathered into a device arena on the context's stream
+ * and copied out on a second stream, so the copies overlap whatever the caller enqueues next (the next load and step of a
+ * double-buffered loop).  The buffers (pinned, for the copies to be asynchronous) are valid after ccake_read_fields_wait;
+ * a second asynchronous read waits on the device, not on the host, for the first one's copies. */
+int ccake_read_fields_async(ccake_ctx* c, int32_t nfields, const int32_t* field_ids, double* const* cols, int64_t capacity);
+int ccake_read_fields_wait(ccake_ctx* c);
+
 /* out (host) = { x0, E, P_1, P_2, P_3, S_tot, N_B, N_S, N_Q, sum m, work, n_out_of_table, max |trace pi|,
  *                n_bad, sum_a N_nb(a), n_out_of_table_total } at the current state (DESIGN.md §"Totals").
  * n_out_of_table counts the particles clamped to the EoS table in the evaluation at the current state;

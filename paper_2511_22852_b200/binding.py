@@ -35,7 +35,7 @@ EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_
            "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep", "ccake_slab_substep_part", "ccake_slab_export_records", "ccake_slab_import_records",
            "ccake_slab_export_migrants", "ccake_slab_import_migrants", "ccake_slab_commit", "ccake_slab_info", "ccake_slab_gids",
            "ccake_step",
-           "ccake_synchronize", "ccake_read_fields", "ccake_conserved_totals", "ccake_read_neighbors",
+           "ccake_synchronize", "ccake_read_fields", "ccake_read_fields_async", "ccake_read_fields_wait", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
            "ccake_measure_fp64_peak", "ccake_last_error"]
 
@@ -96,6 +96,8 @@ def lib():
         L.ccake_step.argtypes = [vp, i32]
         L.ccake_synchronize.argtypes = [vp]
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
+        L.ccake_read_fields_async.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64]
+        L.ccake_read_fields_wait.argtypes = [vp]
         L.ccake_conserved_totals.argtypes = [vp, C.POINTER(C.c_double)]
         L.ccake_read_neighbors.argtypes = [vp, vp, vp, vp, i64]
         L.ccake_neighbor_hash.argtypes = [vp, vp, i64]
@@ -293,6 +295,18 @@ class Ccake:
             space = trip[0][1]
         self._chk(lib().ccake_read_fields(self._h, len(ids), idarr, ptrs, self.n, space), "ccake_read_fields")
         return dict(zip(ids, bufs))
+
+    def read_fields_async(self, ids, out):
+        """ccake_read_fields_async into pinned host tensors / arrays `out`; valid after read_fields_wait()."""
+        ids = list(ids)
+        idarr = (C.c_int32 * len(ids))(*ids)
+        trip = [_ptr(b) for b in out]
+        assert all(t[1] == HOST for t in trip)
+        ptrs = (C.c_void_p * len(ids))(*[t[0] for t in trip])
+        self._chk(lib().ccake_read_fields_async(self._h, len(ids), idarr, ptrs, self.n), "ccake_read_fields_async")
+
+    def read_fields_wait(self):
+        self._chk(lib().ccake_read_fields_wait(self._h), "ccake_read_fields_wait")
 
     def conserved_totals(self):
         out = (C.c_double * 16)()

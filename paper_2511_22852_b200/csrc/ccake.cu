@@ -62,6 +62,12 @@ struct ccake_ctx {
   double* theta = nullptr;
   double* scratch = nullptr;    /* N doubles: staging of ccake_read_neighbors */
   double* stage = nullptr;      /* STAGE_FIELDS x npad doubles: staging of ccake_read_fields into host buffers (on first use) */
+  /* ccake_read_fields_async: all requested fields gathered into one arena, copied out on a second stream */
+  double* stage_all = nullptr;
+  int stage_all_fields = 0;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_gathered = nullptr, ev_copied = nullptr;
+  bool read_pending = false;
   double* src = nullptr;        /* 7 x npad, original order: I^mu, I_q of ccake_set_sources (allocated on first use) */
   bool has_src = false;
   Sorted so;
@@ -144,6 +150,8 @@ void free_particles(ccake_ctx* c) {
   cudaFree(c->theta); c->theta = nullptr;
   cudaFree(c->scratch); c->scratch = nullptr;
   cudaFree(c->stage); c->stage = nullptr;
+  if (c->read_pending) { cudaEventSynchronize(c->ev_copied); c->read_pending = false; }
+  cudaFree(c->stage_all); c->stage_all = nullptr; c->stage_all_fields = 0;
   cudaFree(c->src); c->src = nullptr; c->has_src = false;
   cudaFree(c->gid); c->gid = nullptr; cudaFree(c->gid_new); c->gid_new = nullptr;
   cudaFree(c->slot_of); c->slot_of = nullptr;
@@ -701,6 +709,7 @@ int ccake_destroy(ccake_ctx* c) {
   cudaFree(c->grid);
   cudaFree(c->status);
   cudaFree(c->x0_dev);
+  if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_gathered); cudaEventDestroy(c->ev_copied); }
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   delete c;
   return CCAKE_OK;
@@ -1463,8 +1472,8 @@ int ccake_synchronize(ccake_ctx* c) {
   return CCAKE_OK;
 }
 
-int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double* const* cols, int64_t capacity,
-                      int32_t memspace) {
+static int read_fields_impl(ccake_ctx* c, int32_t nfields, const int32_t* ids, double* const* cols, int64_t capacity,
+                            int32_t memspace, bool sync_at_end) {
   if (!c) return CCAKE_EINVAL;
   if (nfields <= 0 || !ids || !cols || (memspace != 0 && memspace != 1)) { c->err = "bad arguments to ccake_read_fields"; return CCAKE_EINVAL; }
   if (!c->loaded) { c->err = "read before load"; return CCAKE_ESTATE; }
@@ -1552,7 +1561,55 @@ int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double*
       if (k % STAGE_FIELDS == STAGE_FIELDS - 1) CK(cudaStreamSynchronize(st));     /* the arena is reused by the next batch */
     }
   }
-  CK(cudaStreamSynchronize(st));
+  if (sync_at_end) CK(cudaStreamSynchronize(st));
+  return CCAKE_OK;
+}
+
+int ccake_read_fields(ccake_ctx* c, int32_t nfields, const int32_t* ids, double* const* cols, int64_t capacity,
+                      int32_t memspace) {
+  return read_fields_impl(c, nfields, ids, cols, capacity, memspace, true);
+}
+
+int ccake_read_fields_async(ccake_ctx* c, int32_t nfields, const int32_t* ids, double* const* cols, int64_t capacity) {
+  if (!c) return CCAKE_EINVAL;
+  if (nfields <= 0 || !ids || !cols) { c->err = "bad arguments to ccake_read_fields_async"; return CCAKE_EINVAL; }
+  if (!c->loaded) { c->err = "read before load"; return CCAKE_ESTATE; }
+  if (capacity < c->N) { c->err = "capacity < n"; return CCAKE_EINVAL; }
+  for (int k = 0; k < nfields; ++k) if (!cols[k]) { c->err = "null column"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  const int64_t np = c->npad, N = c->N;
+  if (!c->copy_stream) {
+    CK(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&c->ev_gathered, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming));
+  }
+  if (c->stage_all_fields < nfields) {
+    if (c->read_pending) { CK(cudaEventSynchronize(c->ev_copied)); c->read_pending = false; }
+    cudaFree(c->stage_all); c->stage_all = nullptr; c->stage_all_fields = 0;
+    CK(cudaMalloc(&c->stage_all, sizeof(double) * np * nfields));
+    c->stage_all_fields = nfields;
+  }
+  /* the arena of the previous asynchronous read must have left before it is overwritten: the stream waits, not the host */
+  if (c->read_pending) CK(cudaStreamWaitEvent(c->stream, c->ev_copied, 0));
+  std::vector<double*> dev(nfields);
+  for (int k = 0; k < nfields; ++k) dev[k] = c->stage_all + (int64_t)k * np;
+  const int rc = read_fields_impl(c, nfields, ids, dev.data(), np, CCAKE_DEVICE, false);
+  if (rc) return rc;
+  CK(cudaEventRecord(c->ev_gathered, c->stream));
+  CK(cudaStreamWaitEvent(c->copy_stream, c->ev_gathered, 0));
+  for (int k = 0; k < nfields; ++k)
+    CK(cudaMemcpyAsync(cols[k], dev[k], sizeof(double) * N, cudaMemcpyDeviceToHost, c->copy_stream));
+  CK(cudaEventRecord(c->ev_copied, c->copy_stream));
+  c->read_pending = true;
+  return CCAKE_OK;
+}
+
+int ccake_read_fields_wait(ccake_ctx* c) {
+  if (!c) return CCAKE_EINVAL;
+  if (!c->read_pending) return CCAKE_OK;
+  CK(cudaSetDevice(c->device));
+  CK(cudaEventSynchronize(c->ev_copied));
+  c->read_pending = false;
   return CCAKE_OK;
 }
 

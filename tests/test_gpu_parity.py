@@ -222,6 +222,31 @@ def test_graph_replay_equals_direct_launches(name):
     ga.close(); gb.close()
 
 
+def test_async_read_equals_blocking_read():
+    """ccake_read_fields_async + wait return what ccake_read_fields returns, also with steps enqueued in between and with two
+    reads in flight one after the other."""
+    import torch
+    w = WORKLOADS["C4_small"]()
+    stream = torch.cuda.Stream()
+    g = B.from_workload(w, stream=stream.cuda_stream)
+    ids = state_ids(w.params) + [B.T, B.SIGMA_STAR]
+    bufs = [[torch.empty(w.n, dtype=torch.float64).pin_memory() for _ in ids] for _ in range(2)]
+    g.step(2)
+    g.read_fields_async(ids, bufs[0])
+    g.step(1)                                                # enqueued while the copies of the first read run
+    g.read_fields_async(ids, bufs[1])
+    g.read_fields_wait()
+    ref1 = g.read_fields(ids)
+    for k, b in zip(ids, bufs[1]):
+        assert np.array_equal(b.numpy(), ref1[k]), k
+    g2 = B.from_workload(w)
+    g2.step(2)
+    ref0 = g2.read_fields(ids)
+    for k, b in zip(ids, bufs[0]):
+        assert np.array_equal(b.numpy(), ref0[k]), k
+    g.close(); g2.close()
+
+
 def test_full_size_c2():
     """BASELINE.json configs[1] at full size (40,000 particles, 100x32^3x8 table), whole workload on both sides:
     one evaluation, then 20 RK2 steps."""
