@@ -206,7 +206,8 @@ int ccake_slab_import_records(ccake_ctx* c, int32_t side, const double* buf, int
 /* After the last substep: the owned particles that left [lo, hi) through `side`, as a message. */
 int ccake_slab_export_migrants(ccake_ctx* c, int32_t side, double* buf, int64_t buf_cap, int64_t* count);
 int ccake_slab_import_migrants(ccake_ctx* c, int32_t side, const double* buf, int64_t buf_cap, int64_t count);
-/* Rebuild the owned set: stayers (store order) + arrivals from the low side + arrivals from the high side; ghosts dropped. */
+/* Rebuild the owned set: stayers (store order) + arrivals from the low side + arrivals from the high side; ghosts dropped.
+ * The load indices change, so sources set with ccake_set_sources are switched off and have to be set again. */
 int ccake_slab_commit(ccake_ctx* c, int64_t* n_own_new);
 /* out = { n_own, ghosts from the low side, ghosts from the high side, capacity } */
 int ccake_slab_info(ccake_ctx* c, int64_t out[4]);

@@ -1393,6 +1393,7 @@ int ccake_slab_commit(ccake_ctx* c, int64_t* n_own_new) {
   c->n_ghost[0] = c->n_ghost[1] = 0; c->halo_cnt[0] = c->halo_cnt[1] = 0; c->mig_in[0] = c->mig_in[1] = 0;
   c->inv_valid = false;
   c->derived_valid = false;
+  c->has_src = false;                   /* source columns are by load index, which the commit has just renumbered */
   if (n_own_new) *n_own_new = nnew;
   return launch_check(c, "slab_commit");
 }
