@@ -110,6 +110,16 @@ int ccake_destroy(ccake_ctx* c);
 int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* field_ids,
                          const double* const* cols, int32_t memspace);
 
+/* The same in two halves, for a loop over independent particle sets (events): ccake_stage_particles starts copying the
+ * HOST columns (pinned, for the copies to be asynchronous; they must stay untouched until ccake_load_staged has been
+ * called) into a staging arena on a copy stream of its own and returns at once — the copies overlap the steps of the
+ * resident set and the read-back of ccake_read_fields_async.  ccake_load_staged installs the staged set exactly as
+ * ccake_load_particles would: device-side copies on the context's stream that wait, on the device, for the staged
+ * columns; when the particle count equals the resident one it does not wait on the host at all.  One set can be staged
+ * at a time: staging again before ccake_load_staged replaces it.  ESTATE: ccake_load_staged with nothing staged. */
+int ccake_stage_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* field_ids, const double* const* cols);
+int ccake_load_staged(ccake_ctx* c);
+
 /* Load the offline-inverted EoS table (PAPER.md :583-593).  Axis 0 is s; axes 1..3 are B, S, Q, each either the
  * density n_q (axis_kind 0) or the ratio n_q / s (axis_kind 1).  axes[k] = dims[k] strictly increasing node
  * values (any spacing, e.g. the paper's log-decade pattern).  data is row-major [d0][d1][d2][d3][ncols] with

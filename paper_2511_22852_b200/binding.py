@@ -35,7 +35,7 @@ EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_
            "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep", "ccake_slab_substep_part", "ccake_slab_export_records", "ccake_slab_import_records",
            "ccake_slab_export_migrants", "ccake_slab_import_migrants", "ccake_slab_commit", "ccake_slab_info", "ccake_slab_gids",
            "ccake_step",
-           "ccake_synchronize", "ccake_read_fields", "ccake_read_fields_async", "ccake_read_fields_wait", "ccake_conserved_totals", "ccake_read_neighbors",
+           "ccake_synchronize", "ccake_read_fields", "ccake_read_fields_async", "ccake_read_fields_wait", "ccake_stage_particles", "ccake_load_staged", "ccake_conserved_totals", "ccake_read_neighbors",
            "ccake_neighbor_hash", "ccake_kernel_times", "ccake_enable_timing", "ccake_launch_count",
            "ccake_measure_fp64_peak", "ccake_last_error"]
 
@@ -98,6 +98,8 @@ def lib():
         L.ccake_read_fields.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64, i32]
         L.ccake_read_fields_async.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i64]
         L.ccake_read_fields_wait.argtypes = [vp]
+        L.ccake_stage_particles.argtypes = [vp, i64, i32, C.POINTER(i32), C.POINTER(vp)]
+        L.ccake_load_staged.argtypes = [vp]
         L.ccake_conserved_totals.argtypes = [vp, C.POINTER(C.c_double)]
         L.ccake_read_neighbors.argtypes = [vp, vp, vp, vp, i64]
         L.ccake_neighbor_hash.argtypes = [vp, vp, i64]
@@ -187,6 +189,22 @@ class Ccake:
         ptrs = (C.c_void_p * len(ids))(*[t[0] for t in trip])
         self._chk(lib().ccake_load_particles(self._h, n, len(ids), idarr, ptrs, spaces.pop()), "ccake_load_particles")
         self.n = n
+
+    def stage_particles(self, fields: dict):
+        """ccake_stage_particles: start the host -> device copies of the next particle set (pinned host columns)."""
+        ids = list(fields.keys())
+        trip = [_ptr(fields[k]) for k in ids]
+        assert all(t[1] == HOST for t in trip)
+        n = int(trip[0][2].shape[0])
+        assert all(int(t[2].shape[0]) == n for t in trip)
+        idarr = (C.c_int32 * len(ids))(*ids)
+        ptrs = (C.c_void_p * len(ids))(*[t[0] for t in trip])
+        self._chk(lib().ccake_stage_particles(self._h, n, len(ids), idarr, ptrs), "ccake_stage_particles")
+        self._staged_n = n
+
+    def load_staged(self):
+        self._chk(lib().ccake_load_staged(self._h), "ccake_load_staged")
+        self.n = self._staged_n
 
     def load_eos_table(self, axes, axis_kind, col_ids, data):
         ax = [np.ascontiguousarray(a, dtype=np.float64) for a in axes]

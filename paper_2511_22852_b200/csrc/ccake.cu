@@ -68,6 +68,13 @@ struct ccake_ctx {
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_gathered = nullptr, ev_copied = nullptr;
   bool read_pending = false;
+  /* ccake_stage_particles: the next particle set, copied in on a third stream while the resident one is stepped */
+  double* in_stage = nullptr;
+  int64_t in_stage_len = 0, in_n = 0;
+  std::vector<int32_t> in_ids;
+  cudaStream_t h2d_stream = nullptr;
+  cudaEvent_t ev_staged = nullptr, ev_consumed = nullptr;
+  bool in_pending = false, in_consumed_rec = false;
   double* src = nullptr;        /* 7 x npad, original order: I^mu, I_q of ccake_set_sources (allocated on first use) */
   bool has_src = false;
   Sorted so;
@@ -710,6 +717,11 @@ int ccake_destroy(ccake_ctx* c) {
   cudaFree(c->status);
   cudaFree(c->x0_dev);
   if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_gathered); cudaEventDestroy(c->ev_copied); }
+  if (c->h2d_stream) {
+    cudaStreamSynchronize(c->h2d_stream);
+    cudaStreamDestroy(c->h2d_stream); cudaEventDestroy(c->ev_staged); cudaEventDestroy(c->ev_consumed);
+  }
+  cudaFree(c->in_stage);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   delete c;
   return CCAKE_OK;
@@ -849,6 +861,59 @@ int ccake_load_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t
   if (c->loaded && !c->slab && n == c->N && c->cap == n) return reload_particles(c, nfields, ids, cols, memspace);
   c->slab = false;
   return load_impl(c, n, n, nfields, ids, cols, memspace);
+}
+
+int ccake_stage_particles(ccake_ctx* c, int64_t n, int32_t nfields, const int32_t* ids, const double* const* cols) {
+  if (!c) return CCAKE_EINVAL;
+  if (n <= 0 || nfields <= 0 || !ids || !cols || n > 2000000000LL) { c->err = "bad arguments to ccake_stage_particles"; return CCAKE_EINVAL; }
+  for (int k = 0; k < nfields; ++k)
+    if (ids[k] < 0 || ids[k] >= NSTATE || !cols[k]) { c->err = "bad field id in stage"; return CCAKE_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  if (!c->h2d_stream) {
+    CK(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&c->ev_staged, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&c->ev_consumed, cudaEventDisableTiming));
+  }
+  if (c->in_stage_len < n * nfields) {
+    CK(cudaStreamSynchronize(c->h2d_stream));
+    if (c->in_consumed_rec) CK(cudaEventSynchronize(c->ev_consumed));
+    cudaFree(c->in_stage); c->in_stage = nullptr; c->in_stage_len = 0;
+    CK(cudaMalloc(&c->in_stage, sizeof(double) * n * nfields));
+    c->in_stage_len = n * nfields;
+  }
+  /* the arena may still be read by the device-side copies of the previous ccake_load_staged: the copy stream waits for
+     them, not the host */
+  if (c->in_consumed_rec) CK(cudaStreamWaitEvent(c->h2d_stream, c->ev_consumed, 0));
+  for (int k = 0; k < nfields; ++k)
+    CK(cudaMemcpyAsync(c->in_stage + (int64_t)k * n, cols[k], sizeof(double) * n, cudaMemcpyHostToDevice, c->h2d_stream));
+  CK(cudaEventRecord(c->ev_staged, c->h2d_stream));
+  c->in_ids.assign(ids, ids + nfields);
+  c->in_n = n;
+  c->in_pending = true;
+  return CCAKE_OK;
+}
+
+int ccake_load_staged(ccake_ctx* c) {
+  if (!c) return CCAKE_EINVAL;
+  if (!c->in_pending) { c->err = "ccake_load_staged without ccake_stage_particles"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  const int64_t n = c->in_n;
+  const int nfields = (int)c->in_ids.size();
+  std::vector<const double*> dev(nfields);
+  for (int k = 0; k < nfields; ++k) dev[k] = c->in_stage + (int64_t)k * n;
+  CK(cudaStreamWaitEvent(c->stream, c->ev_staged, 0));
+  int rc;
+  if (c->loaded && !c->slab && n == c->N && c->cap == n) {
+    rc = reload_particles(c, nfields, c->in_ids.data(), dev.data(), CCAKE_DEVICE);    /* nothing here waits on the host */
+  } else {
+    CK(cudaStreamSynchronize(c->stream));
+    c->slab = false;
+    rc = load_impl(c, n, n, nfields, c->in_ids.data(), dev.data(), CCAKE_DEVICE);
+  }
+  CK(cudaEventRecord(c->ev_consumed, c->stream));
+  c->in_consumed_rec = true;
+  c->in_pending = false;
+  return rc;
 }
 
 int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis_kind[4], const double* const axes[4],

@@ -247,6 +247,55 @@ def test_async_read_equals_blocking_read():
     g.close(); g2.close()
 
 
+def test_staged_load_equals_blocking_load():
+    """ccake_stage_particles + ccake_load_staged install what ccake_load_particles installs: the same results bit for bit,
+    with the copies of the next set in flight while the resident one is stepped and read back, with a set of another size
+    (the path that reallocates), and ESTATE with nothing staged."""
+    import torch
+    w = WORKLOADS["C4_small"]()
+    stream = torch.cuda.Stream()
+    g = B.from_workload(w, stream=stream.cuda_stream)
+    ids = state_ids(w.params) + [B.T, B.SIGMA_STAR]
+    g.step(2)
+    ref = g.read_fields(ids)
+    with pytest.raises(B.CcakeError):
+        g.load_staged()
+    rng = np.random.default_rng(5)
+    fields2 = {k: v.copy() for k, v in w.fields.items()}
+    fields2[B.S] = fields2[B.S] * (1.0 + 0.05 * rng.uniform(-1.0, 1.0, w.n))        # a second, different event
+    pin = [{k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in f.items()} for f in (w.fields, fields2)]
+    bufs = [[torch.empty(w.n, dtype=torch.float64).pin_memory() for _ in ids] for _ in range(3)]
+    g.stage_particles(pin[0])
+    for it in range(3):                                      # events 0, 1, 0: load, stage the next one, step, read back
+        g.load_staged()
+        if it < 2:
+            g.stage_particles(pin[(it + 1) % 2])
+        g.step(2)
+        g.read_fields_async(ids, bufs[it])
+    g.read_fields_wait()
+    g.synchronize()
+    g2 = B.from_workload(w)
+    g2.load_particles(fields2)
+    g2.step(2)
+    ref2 = g2.read_fields(ids)
+    for k, b0, b1, b2 in zip(ids, *bufs):
+        assert np.array_equal(b0.numpy(), ref[k]), k
+        assert np.array_equal(b1.numpy(), ref2[k]), k
+        assert np.array_equal(b2.numpy(), ref[k]), k
+    # another particle count: the staged set goes through the allocating load
+    m = w.n // 2
+    half = {k: torch.from_numpy(np.ascontiguousarray(v[:m])).pin_memory() for k, v in w.fields.items()}
+    g.stage_particles(half)
+    g.load_staged()
+    g.step(1)
+    g2.load_particles({k: v[:m] for k, v in w.fields.items()})
+    g2.step(1)
+    a, b = g.read_fields(ids), g2.read_fields(ids)
+    for k in ids:
+        assert a[k].shape == (m,) and np.array_equal(a[k], b[k]), k
+    g.close(); g2.close()
+
+
 def test_full_size_c2():
     """BASELINE.json configs[1] at full size (40,000 particles, 100x32^3x8 table), whole workload on both sides:
     one evaluation, then 20 RK2 steps."""
