@@ -237,7 +237,7 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
   const int D = c->P.dim;
   cudaStream_t st = c->stream;
   bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, st>>>(Ycur, np, N, D, c->bbox_partial);
-  bbox_final_kernel<<<1, 32, 0, st>>>(c->bbox_partial, c->bbox_blocks, D, c->P.h, c->max_cells, c->grid);
+  bbox_final_kernel<<<1, BBOX_FINAL_THREADS, 0, st>>>(c->bbox_partial, c->bbox_blocks, D, c->P.h, c->max_cells, c->grid);
   cell_hash_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->grid, c->key[0], c->val[0]);
   int cur = 0;
   for (int pass = 0; pass < c->passes; ++pass) {
@@ -824,7 +824,7 @@ static int load_impl(ccake_ctx* c, int64_t n, int64_t cap, int32_t nfields, cons
   CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
   /* size the radix-sort key from the bounding box at load; the device coarsens the grid if the system outgrows it */
   bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, c->stream>>>(c->Y[0], np, n, c->P.dim, c->bbox_partial);
-  bbox_final_kernel<<<1, 32, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 22, c->grid);
+  bbox_final_kernel<<<1, BBOX_FINAL_THREADS, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 22, c->grid);
   Grid g;
   CK(cudaMemcpyAsync(&g, c->grid, sizeof(Grid), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
@@ -958,11 +958,24 @@ int ccake_load_eos_table(ccake_ctx* c, const int32_t dims[4], const int32_t axis
   drop_graphs(c);
   free_table(c);
   CK(cudaMalloc(&c->tb_axes, sizeof(double) * nax));
-  CK(cudaMalloc(&c->tb_data, sizeof(double) * nodes * ncols));
+  CK(cudaMalloc(&c->tb_data, sizeof(double) * nodes * TB_STRIDE));
   CK(cudaMemcpyAsync(c->tb_axes, hax.data(), sizeof(double) * nax, cudaMemcpyHostToDevice, c->stream));
-  CK(cudaMemcpyAsync(c->tb_data, data, sizeof(double) * nodes * ncols,
-                     memspace == CCAKE_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
-  CK(cudaStreamSynchronize(c->stream));
+  {
+    /* the resident copy holds, per node, the CCAKE_NCOLS_MAX columns in the order of their ids (absent ones 0) in
+       TB_STRIDE doubles, so that the lookup reads a node with 16-byte loads and without a column map */
+    const double* src = data;
+    double* tmp = nullptr;
+    if (memspace == CCAKE_HOST) {
+      if (cudaMalloc(&tmp, sizeof(double) * nodes * ncols) != cudaSuccess) { cudaGetLastError(); c->err = "table allocation"; return CCAKE_ENOMEM; }
+      CK(cudaMemcpyAsync(tmp, data, sizeof(double) * nodes * ncols, cudaMemcpyHostToDevice, c->stream));
+      src = tmp;
+    }
+    table_pack_kernel<<<nblk(nodes * TB_STRIDE, 256), 256, 0, c->stream>>>(src, ncols, nodes, tb, c->tb_data);
+    c->launches += 1;
+    const cudaError_t e = cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    CK(e);
+  }
   {
     int64_t off = 0;
     for (int k = 0; k < 4; ++k) { tb.dims[k] = dims[k]; tb.kind[k] = axis_kind[k]; tb.ax[k] = c->tb_axes + off; off += dims[k]; }

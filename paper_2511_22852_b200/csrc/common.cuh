@@ -92,7 +92,10 @@ struct KParams {
   double kappa_over_T2[9], tau_q_times_T[3], dnmr[8];
 };
 
-/* EoS table descriptor (device pointers) */
+/* EoS table descriptor (device pointers).  data: TB_STRIDE doubles per node, column id c at position c (absent columns 0),
+   nodes in the caller's order (last axis fastest); col_of / ncols describe the caller's layout (table_pack_kernel). */
+constexpr int TB_STRIDE = 12;
+static_assert(TB_STRIDE >= CCAKE_NCOLS_MAX && TB_STRIDE % 2 == 0, "node record");
 struct TableDev {
   int dims[4], kind[4], ncols;
   int col_of[CCAKE_NCOLS_MAX];

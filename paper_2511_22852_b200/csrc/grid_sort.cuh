@@ -52,17 +52,24 @@ bbox_partial_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D
   }
 }
 
-/* one block: reduce the partials (min/max are exact and order-free) and lay out the traversal grid */
+/* one block of BBOX_FINAL_THREADS = 6 warps: reduce the partials (min/max are exact and order-free) and lay out the traversal grid */
+constexpr int BBOX_FINAL_THREADS = 192;
 __global__ void bbox_final_kernel(const double* __restrict__ partial, int nblocks, int D, double h, int max_cells,
                                   Grid* __restrict__ grid) {
   __shared__ double red[6];
-  if (threadIdx.x < 6) {
-    double r = partial[threadIdx.x];
-    for (int b = 1; b < nblocks; ++b) {
-      const double v = partial[b * 6 + threadIdx.x];
-      r = (threadIdx.x < 3) ? fmin(r, v) : fmax(r, v);
+  {
+    /* warp q reduces quantity q (0..2: minima, 3..5: maxima), its lanes striding over the blocks */
+    const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double r = partial[q];
+    for (int b = lane; b < nblocks; b += 32) {
+      const double v = partial[b * 6 + q];
+      r = (q < 3) ? fmin(r, v) : fmax(r, v);
     }
-    red[threadIdx.x] = r;
+    for (int o = 16; o > 0; o >>= 1) {
+      const double v = __shfl_xor_sync(0xffffffffu, r, o);
+      r = (q < 3) ? fmin(r, v) : fmax(r, v);
+    }
+    if (lane == 0) red[q] = r;
   }
   __syncthreads();
   if (threadIdx.x == 0) {

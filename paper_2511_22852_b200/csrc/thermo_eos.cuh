@@ -27,6 +27,16 @@ __device__ inline int axis_cell(const double* __restrict__ ax, int n, double x) 
   return i;
 }
 
+/* caller's table [node][ncols] -> resident copy [node][TB_STRIDE] (TableDev) */
+__global__ void table_pack_kernel(const double* __restrict__ src, int ncols, int64_t nodes, TableDev tb, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nodes * TB_STRIDE) return;
+  const int64_t node = i / TB_STRIDE;
+  const int c = (int)(i - node * TB_STRIDE);
+  const int k = (c < CCAKE_NCOLS_MAX) ? tb.col_of[c] : -1;
+  dst[i] = (k >= 0) ? src[node * ncols + k] : 0.0;
+}
+
 __device__ inline ThermoOut eos_table_lookup(const TableDev& tb, double s, const double n[NQ]) {
   ThermoOut th;
   th.oob = 0;
@@ -47,10 +57,9 @@ __device__ inline ThermoOut eos_table_lookup(const TableDev& tb, double s, const
     const double lo = ax[i], hi = ax[i + 1];
     t[k] = (xv - lo) / (hi - lo);
   }
-  double out[CCAKE_NCOLS_MAX];
-  for (int c = 0; c < CCAKE_NCOLS_MAX; ++c) out[c] = 0.0;
-  const int nc = tb.ncols;
-  /* 16 nodes; the two nodes along the innermost axis are adjacent in memory (2 * ncols doubles) */
+  double out[TB_STRIDE];
+  for (int c = 0; c < TB_STRIDE; ++c) out[c] = 0.0;
+  /* 16 nodes; the two nodes along the innermost axis are adjacent in memory (2 * TB_STRIDE doubles, 16-byte loads) */
   for (int b0 = 0; b0 < 2; ++b0)
     for (int b1 = 0; b1 < 2; ++b1)
       for (int b2 = 0; b2 < 2; ++b2) {
@@ -59,11 +68,13 @@ __device__ inline ThermoOut eos_table_lookup(const TableDev& tb, double s, const
         const double w2 = b2 ? t[2] : 1.0 - t[2];
         const double w012 = (w0 * w1) * w2;
         const int64_t node = (((int64_t)(i0[0] + b0) * tb.dims[1] + (i0[1] + b1)) * tb.dims[2] + (i0[2] + b2)) * tb.dims[3] + i0[3];
-        const double* __restrict__ p0 = tb.data + node * nc;
+        const double2* __restrict__ p0 = reinterpret_cast<const double2*>(tb.data + node * TB_STRIDE);
         const double wl = w012 * (1.0 - t[3]), wh = w012 * t[3];
-        for (int c = 0; c < CCAKE_NCOLS_MAX; ++c) {
-          const int col = tb.col_of[c];
-          if (col >= 0) { out[c] += wl * __ldg(p0 + col); out[c] += wh * __ldg(p0 + nc + col); }
+#pragma unroll
+        for (int u = 0; u < TB_STRIDE / 2; ++u) {
+          const double2 lo = __ldg(p0 + u), hi = __ldg(p0 + TB_STRIDE / 2 + u);
+          out[2 * u] += wl * lo.x; out[2 * u] += wh * hi.x;
+          out[2 * u + 1] += wl * lo.y; out[2 * u + 1] += wh * hi.y;
         }
       }
   th.T = out[CCAKE_COL_T];
