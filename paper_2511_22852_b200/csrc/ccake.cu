@@ -47,6 +47,7 @@ struct ccake_ctx {
   Grid* grid = nullptr;
   Status* status = nullptr;
   double* bbox_partial = nullptr;
+  unsigned int* bbox_ticket = nullptr;     /* bbox_kernel: blocks finished so far (0 between launches) */
   int bbox_blocks = 0;
   double *tot_partial = nullptr, *tot_out = nullptr;
   int tot_blocks = 0;
@@ -236,8 +237,7 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
   const int64_t N = c->N, np = c->npad;
   const int D = c->P.dim;
   cudaStream_t st = c->stream;
-  bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, st>>>(Ycur, np, N, D, c->bbox_partial);
-  bbox_final_kernel<<<1, BBOX_FINAL_THREADS, 0, st>>>(c->bbox_partial, c->bbox_blocks, D, c->P.h, c->max_cells, c->grid);
+  bbox_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, st>>>(Ycur, np, N, D, c->bbox_partial, c->bbox_ticket, c->P.h, c->max_cells, c->grid);
   cell_hash_kernel<<<nblk(N, 256), 256, 0, st>>>(Ycur, np, N, D, c->grid, c->key[0], c->val[0]);
   int cur = 0;
   for (int pass = 0; pass < c->passes; ++pass) {
@@ -260,10 +260,9 @@ int build_cells(ccake_ctx* c, double*& Ycur, bool reorder) {
     std::swap(c->orig[0], c->orig[1]);
     c->inv_valid = false;
     Ycur = c->Y[0];
-    iota_kernel<<<nblk(N, 256), 256, 0, st>>>(c->so.perm, N);
-    c->launches += 2;
+    c->launches += 1;
   }
-  c->launches += 4 + 4 * c->passes;
+  c->launches += 3 + 4 * c->passes;
   return launch_check(c, "build_cells");
 }
 
@@ -694,9 +693,11 @@ int ccake_create(const ccake_params* p, ccake_ctx** out) {
   if (p->coords == 1 && p->dim == 2) on(CCAKE_WORK);
   c->field_mask = m;
   if (cudaMalloc(&c->grid, sizeof(Grid)) != cudaSuccess || cudaMalloc(&c->status, sizeof(Status)) != cudaSuccess ||
-      cudaMalloc(&c->x0_dev, sizeof(double)) != cudaSuccess) {
+      cudaMalloc(&c->x0_dev, sizeof(double)) != cudaSuccess || cudaMalloc(&c->bbox_ticket, sizeof(unsigned int)) != cudaSuccess ||
+      cudaMemset(c->bbox_ticket, 0, sizeof(unsigned int)) != cudaSuccess) {
     cudaFree(c->grid);
     cudaFree(c->status);
+    cudaFree(c->x0_dev);
     delete c;
     return CCAKE_ENOMEM;
   }
@@ -716,6 +717,7 @@ int ccake_destroy(ccake_ctx* c) {
   cudaFree(c->grid);
   cudaFree(c->status);
   cudaFree(c->x0_dev);
+  cudaFree(c->bbox_ticket);
   if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->ev_gathered); cudaEventDestroy(c->ev_copied); }
   if (c->h2d_stream) {
     cudaStreamSynchronize(c->h2d_stream);
@@ -823,8 +825,7 @@ static int load_impl(ccake_ctx* c, int64_t n, int64_t cap, int32_t nfields, cons
   iota_kernel<<<nblk(n, 256), 256, 0, c->stream>>>(c->orig[0], n);
   CK(cudaMemsetAsync(c->status, 0, sizeof(Status), c->stream));
   /* size the radix-sort key from the bounding box at load; the device coarsens the grid if the system outgrows it */
-  bbox_partial_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, c->stream>>>(c->Y[0], np, n, c->P.dim, c->bbox_partial);
-  bbox_final_kernel<<<1, BBOX_FINAL_THREADS, 0, c->stream>>>(c->bbox_partial, c->bbox_blocks, c->P.dim, c->P.h, 1 << 22, c->grid);
+  bbox_kernel<<<c->bbox_blocks, BBOX_THREADS, 0, c->stream>>>(c->Y[0], np, n, c->P.dim, c->bbox_partial, c->bbox_ticket, c->P.h, 1 << 22, c->grid);
   Grid g;
   CK(cudaMemcpyAsync(&g, c->grid, sizeof(Grid), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));

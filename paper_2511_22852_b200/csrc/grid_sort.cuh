@@ -25,44 +25,16 @@ __device__ inline double warp_max(double v) {
   return v;
 }
 
-/* partial[block][0..5] = min x,y,z, max x,y,z over the block's grid-stride share */
-__global__ void __launch_bounds__(BBOX_THREADS)
-bbox_partial_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D, double* __restrict__ partial) {
-  double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    for (int k = 0; k < 3; ++k) {
-      if (k < D) {
-        const double v = Y[(CCAKE_R1 + k) * npad + i];
-        lo[k] = fmin(lo[k], v);
-        hi[k] = fmax(hi[k], v);
-      }
-    }
-  }
-  __shared__ double sm[6][BBOX_THREADS / 32];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (int k = 0; k < 3; ++k) {
-    const double a = warp_min(lo[k]), b = warp_max(hi[k]);
-    if (lane == 0) { sm[k][w] = a; sm[3 + k][w] = b; }
-  }
-  __syncthreads();
-  if (threadIdx.x < 6) {
-    double r = sm[threadIdx.x][0];
-    for (int j = 1; j < BBOX_THREADS / 32; ++j) r = (threadIdx.x < 3) ? fmin(r, sm[threadIdx.x][j]) : fmax(r, sm[threadIdx.x][j]);
-    partial[blockIdx.x * 6 + threadIdx.x] = r;
-  }
-}
-
-/* one block of BBOX_FINAL_THREADS = 6 warps: reduce the partials (min/max are exact and order-free) and lay out the traversal grid */
-constexpr int BBOX_FINAL_THREADS = 192;
-__global__ void bbox_final_kernel(const double* __restrict__ partial, int nblocks, int D, double h, int max_cells,
-                                  Grid* __restrict__ grid) {
+/* the threads of ONE block (at least 6 warps): reduce the partials (min/max are exact and order-free) and lay out the
+   traversal grid */
+__device__ __forceinline__ void bbox_finish(const double* partial, int nblocks, int D, double h, int max_cells, Grid* __restrict__ grid) {
   __shared__ double red[6];
-  {
+  if (threadIdx.x < 192) {
     /* warp q reduces quantity q (0..2: minima, 3..5: maxima), its lanes striding over the blocks */
     const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double r = partial[q];
+    double r = __ldcg(partial + q);                    /* written by other blocks of this launch */
     for (int b = lane; b < nblocks; b += 32) {
-      const double v = partial[b * 6 + q];
+      const double v = __ldcg(partial + b * 6 + q);
       r = (q < 3) ? fmin(r, v) : fmax(r, v);
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -114,6 +86,46 @@ __global__ void bbox_final_kernel(const double* __restrict__ partial, int nblock
     }
     *grid = g;
   }
+}
+
+/* partial[block][0..5] = min x,y,z, max x,y,z over the block's grid-stride share; the block that finishes last (a ticket
+   counter, left at 0 for the next launch) reduces the partials and writes the grid: one launch for step a1 */
+__global__ void __launch_bounds__(BBOX_THREADS)
+bbox_kernel(const double* __restrict__ Y, int64_t npad, int64_t n, int D, double* partial, unsigned int* __restrict__ ticket,
+            double h, int max_cells, Grid* __restrict__ grid) {
+  double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    for (int k = 0; k < 3; ++k) {
+      if (k < D) {
+        const double v = Y[(CCAKE_R1 + k) * npad + i];
+        lo[k] = fmin(lo[k], v);
+        hi[k] = fmax(hi[k], v);
+      }
+    }
+  }
+  __shared__ double sm[6][BBOX_THREADS / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int k = 0; k < 3; ++k) {
+    const double a = warp_min(lo[k]), b = warp_max(hi[k]);
+    if (lane == 0) { sm[k][w] = a; sm[3 + k][w] = b; }
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    double r = sm[threadIdx.x][0];
+    for (int j = 1; j < BBOX_THREADS / 32; ++j) r = (threadIdx.x < 3) ? fmin(r, sm[threadIdx.x][j]) : fmax(r, sm[threadIdx.x][j]);
+    partial[blockIdx.x * 6 + threadIdx.x] = r;
+  }
+  __shared__ bool last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    if (last) *ticket = 0u;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  bbox_finish(partial, (int)gridDim.x, D, h, max_cells, grid);
 }
 
 /* ------------------------------------------------------------------------------------------ a2 hash ---- */
@@ -274,7 +286,7 @@ scan_totals_kernel(uint32_t* __restrict__ chunk_tot, int nchunks) {
 /* pass 3 of 3: stable scatter.  Keys of a tile are visited in rounds of SORT_THREADS consecutive keys; within a
    round the rank of a key among equal digits is (keys of earlier rounds) + (equal digits in lower warps) +
    (equal digits in lower lanes), which preserves the input order. */
-__global__ void __launch_bounds__(SORT_THREADS)
+__global__ void __launch_bounds__(SORT_THREADS, 4)
 radix_scatter_kernel(const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, int64_t n, int shift,
                      int ntiles, const uint32_t* __restrict__ hist, const uint32_t* __restrict__ chunk_off,
                      uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out) {
@@ -289,11 +301,22 @@ radix_scatter_kernel(const uint32_t* __restrict__ key_in, const uint32_t* __rest
   }
   __syncthreads();
   const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+  /* all keys and values of the thread are loaded up front: one memory latency per tile instead of one per round */
+  uint32_t kk[SORT_ITEMS], vv[SORT_ITEMS];
+#pragma unroll
   for (int r = 0; r < SORT_ITEMS; ++r) {
     const int64_t i = base + r * SORT_THREADS + threadIdx.x;
+    kk[r] = 0; vv[r] = 0;
+    if (i < n) { kk[r] = key_in[i]; vv[r] = val_in[i]; }
+  }
+  const int rounds = (int)min((int64_t)SORT_ITEMS, (n - base + SORT_THREADS - 1) / SORT_THREADS);   /* the last tile may be short */
+#pragma unroll
+  for (int r = 0; r < SORT_ITEMS; ++r) {
+    if (r >= rounds) break;
+    const int64_t i = base + r * SORT_THREADS + threadIdx.x;
     const bool ok = i < n;
-    uint32_t k = 0, v = 0, d = 256;
-    if (ok) { k = key_in[i]; v = val_in[i]; d = (k >> shift) & 255u; }
+    const uint32_t k = kk[r], v = vv[r];
+    const uint32_t d = ok ? ((k >> shift) & 255u) : 256u;
     const uint32_t mask = __match_any_sync(0xffffffffu, d);
     const uint32_t rank_w = __popc(mask & ((1u << lane) - 1u));
     if (ok && rank_w == 0) wc[w][d] = __popc(mask);
@@ -333,7 +356,7 @@ __global__ void cell_start_kernel(const uint32_t* __restrict__ key, int64_t n, c
 /* physical reorder of the store at the first substep of a step: dst[f][i] = src[f][perm[i]] for the active
    fields; afterwards the store order IS the sorted order and perm becomes the identity */
 __global__ void reorder_store_kernel(const double* __restrict__ src, double* __restrict__ dst, int64_t npad, int64_t n,
-                                     const uint32_t* __restrict__ perm, uint32_t field_mask,
+                                     uint32_t* __restrict__ perm, uint32_t field_mask,
                                      const uint32_t* __restrict__ orig_src, uint32_t* __restrict__ orig_dst) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -341,6 +364,7 @@ __global__ void reorder_store_kernel(const double* __restrict__ src, double* __r
   for (int f = 0; f < NSTATE; ++f)
     if (field_mask & (1u << f)) dst[f * npad + i] = src[f * npad + a];
   orig_dst[i] = orig_src[a];
+  perm[i] = (uint32_t)i;           /* entry i is read by this thread only */
 }
 
 __global__ void iota_kernel(uint32_t* __restrict__ p, int64_t n) {
