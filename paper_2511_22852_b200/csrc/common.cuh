@@ -93,7 +93,8 @@ struct KParams {
 };
 
 /* EoS table descriptor (device pointers).  data: TB_STRIDE doubles per node, column id c at position c (absent columns 0),
-   nodes in the caller's order (last axis fastest); col_of / ncols describe the caller's layout (table_pack_kernel). */
+   nodes in the caller's order (last axis fastest); col_of / ncols describe the caller's layout (table_pack_kernel).
+   ax[0..3] are consecutive pieces of ONE array (ax[k + 1] = ax[k] + dims[k]). */
 constexpr int TB_STRIDE = 12;
 static_assert(TB_STRIDE >= CCAKE_NCOLS_MAX && TB_STRIDE % 2 == 0, "node record");
 struct TableDev {

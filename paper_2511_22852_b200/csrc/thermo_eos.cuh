@@ -470,11 +470,29 @@ __device__ inline void load_u(const KParams& kp, const Geom& gm, const double* Y
 #ifndef CCAKE_THERMO_MINB
 #define CCAKE_THERMO_MINB 6
 #endif
+#ifndef CCAKE_THERMO_AX_SMEM
+#define CCAKE_THERMO_AX_SMEM 512        /* doubles; 0 = axes read from global memory */
+#endif
 template <int TD, bool TV, bool TF>
 __global__ void __launch_bounds__(128, CCAKE_THERMO_MINB)
 thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x0_off, TableDev tb, const double* __restrict__ Y,
               int64_t npad, Sorted so, Status* __restrict__ status, int on_step, const uint32_t* __restrict__ orig, int64_t n_own) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+#if CCAKE_THERMO_AX_SMEM
+  /* the table axes (one array, TableDev) go to shared memory: the per-axis binary searches are ~22 dependent loads per
+     particle at lane-divergent indices */
+  __shared__ double s_ax[CCAKE_THERMO_AX_SMEM];
+  if (kp.eos_kind == 1) {
+    const int nax = tb.dims[0] + tb.dims[1] + tb.dims[2] + tb.dims[3];
+    if (nax <= CCAKE_THERMO_AX_SMEM) {
+      const double* __restrict__ ax0 = tb.ax[0];
+      for (int j = threadIdx.x; j < nax; j += blockDim.x) s_ax[j] = ax0[j];
+      __syncthreads();
+      int off = 0;
+      for (int k = 0; k < 4; ++k) { tb.ax[k] = s_ax + off; off += tb.dims[k]; }
+    }
+  }
+#endif
   if (i >= n) return;
   const Geom gm = make_geom(kp.coords, *x0_dev + x0_off);      /* the time lives on the device: a captured step replays */
   constexpr int D = TD;
