@@ -24,7 +24,7 @@
  *   - Candidates of a block come from cand_list_kernel (once per substep, global memory, both passes) or, for a
  *     block whose list does not fit there, from a list built inside the pass (interleaved sweeps).  Their AoS
  *     payload records are copied with cp.async, HALF_B at a time and taken with a stride through the list, into a
- *     ring of NSLOT tiles in shared memory (component-major, one-unit skew) whose arrival is tracked by one
+ *     ring of NSLOT tiles (3 in the gradient pass, 6 in the smoothing pass) in shared memory (component-major, one-unit skew) whose arrival is tracked by one
  *     mbarrier per slot; there is no block barrier per tile.
  *   - Per tile and group the warp tests the 128 candidates against the FP32 box of the group's 8 homes (4 per lane,
  *     ballots) and compacts the survivors into a FIFO of slot numbers; quads of 4 candidates are taken from it,
@@ -67,8 +67,11 @@ constexpr int NR32 = HALF_B / 32;            /* candidates a lane tests per tile
 #ifndef CCAKE_PM_NSLOT
 #define CCAKE_PM_NSLOT 3
 #endif
-constexpr int NSLOT = CCAKE_PM_NSLOT;        /* tiles resident in shared memory: the current one and those in flight */
-constexpr int TILE_B = NSLOT * HALF_B;
+#ifndef CCAKE_PM_NSLOT_S
+#define CCAKE_PM_NSLOT_S 6                   /* measured on C4: 3 / 4 / 5 / 6 / 8 slots -> 8.32 / 8.37 / 8.25 / 8.21 / 8.27 ms */
+#endif
+constexpr int NSLOT_G = CCAKE_PM_NSLOT;      /* tiles resident in shared memory: the current one and those in flight (Op::NSLOT) */
+constexpr int NSLOT_S = CCAKE_PM_NSLOT_S;    /* ... of the smoothing pass, whose records are a quarter of the gradient pass's */
 constexpr int RPW = HALF_B / PM_WARPS;       /* records of a tile each warp copies               */
 #ifndef CCAKE_LCAP
 #define CCAKE_LCAP 1536
@@ -170,7 +173,7 @@ struct SmoothOp {
   static constexpr int D = D_;
   static constexpr bool HASH = HASH_;
   static constexpr bool COUNT = true, GIDMAJOR = false;
-  static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3, XO = 0;
+  static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3, XO = 0, NSLOT = NSLOT_S;
   static constexpr int elem(int, int, int n) { return (n <= 4) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
     const double q = g.q;
@@ -269,7 +272,7 @@ struct GradOp {
   static constexpr int eM = make_glayout(D_, VISC, DIFF).M, eP = make_glayout(D_, VISC, DIFF).P, eU = make_glayout(D_, VISC, DIFF).U,
                        eV = make_glayout(D_, VISC, DIFF).V, eB = make_glayout(D_, VISC, DIFF).B, eK = make_glayout(D_, VISC, DIFF).K,
                        eAL = make_glayout(D_, VISC, DIFF).AL;
-  static constexpr int NREC = GREC_D, XO = GREC_X;
+  static constexpr int NREC = GREC_D, XO = GREC_X, NSLOT = NSLOT_G;
   static constexpr int NJ = D, NT = (VISC || DIFF) ? 2 : 1;
   static constexpr int elem(int, int, int) { return ELEM_NONE; }       /* not used: the operands are found by position */
   /* column positions */
@@ -354,7 +357,7 @@ template <int D_>
 struct EpsGradOp {
   static constexpr int D = D_;
   static constexpr bool HASH = false, COUNT = false, GIDMAJOR = false;
-  static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3, XO = 0;
+  static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3, XO = 0, NSLOT = NSLOT_G;
   static constexpr int elem(int, int, int n) { return (n <= 1) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
     const double t = 2.0 - g.q;
@@ -378,6 +381,7 @@ struct EpsGradOp {
 template <class Op> struct PairCfg {
   static constexpr int NR = Op::NREC;
   static constexpr int NU = NR / 2;
+  static constexpr int NSLOT = Op::NSLOT, TILE_B = NSLOT * HALF_B;
   static constexpr int CSTRIDE = TILE_B + 1;
   static constexpr int NSUM = 8 * Op::NT * Op::NJ;          /* sums per home particle */
   static constexpr int SSTRIDE = NSUM + 2;                  /* scratch row of a home in the epilogue (even, skewed) */
@@ -518,6 +522,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   constexpr int D = Op::D;
   constexpr int NU = PairCfg<Op>::NU;
   constexpr int CSTRIDE = PairCfg<Op>::CSTRIDE;
+  constexpr int NSLOT = PairCfg<Op>::NSLOT, TILE_B = PairCfg<Op>::TILE_B;
   constexpr int NW = PM_WARPS, GPW = PM_GPW, NJ = Op::NJ, NT = Op::NT;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* pay = reinterpret_cast<double2*>(smem_raw);                  /* [NU][CSTRIDE] staged records        */
