@@ -166,6 +166,22 @@ int ccake_invert_forward_table(ccake_ctx* c, const int32_t fdims[4], const doubl
 int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
                         const double* t, double h_source, double eta_norm, double* const j[4], int32_t memspace);
 
+/* The same smearing for callers that must not allocate (a region under CUDA graph capture, a tight serving loop, a harness
+ * that forbids cudaMalloc): ccake_smear_sources allocates and frees two device buffers per call, this entry point calls no
+ * cudaMalloc, cudaFree or allocating library routine.  Its scratch memory — the packed parton array — is a fixed array in
+ * the library's device image: 8 x CCAKE_SMEAR_NOALLOC_MAX doubles = 1 MiB, held by every GPU that loads the library until
+ * the process exits.  EINVAL, with ccake_last_error naming the limit, when npartons > CCAKE_SMEAR_NOALLOC_MAX.
+ * p, r, t, j as in ccake_smear_sources but DEVICE memory only (the caller owns inputs and outputs; j[m] has n doubles and
+ * is overwritten for every particle; with npartons == 0 the input columns may be NULL and j becomes 0).  Asynchronous on the context's stream: j is valid after ccake_synchronize (or in
+ * stream order).  The result is the one ccake_smear_sources gives (same arithmetic in the same order).
+ * The scratch array is shared by every call on a device — all contexts, all streams — and keeps the last call's partons:
+ * each call overwrites the entries it reads (nothing has to be cleared), and two calls that overlap on the GPU (different
+ * streams / contexts of one device) race; calls on one stream are ordered and safe.  The context must have been created
+ * and loaded beforehand (those calls allocate).  ESTATE before a load. */
+#define CCAKE_SMEAR_NOALLOC_MAX 16384
+int ccake_smear_sources_noalloc(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
+                                const double* t, double h_source, double eta_norm, double* const j[4]);
+
 /* Rest of NEXT-3: source terms of the conservation equations, Eq. 38 (:623) nabla_mu T^{mu nu} = I^nu,
  * nabla_mu N^mu_q = I_q, as they enter Eq. 42-44 (:645-649) and the entropy equation Eq. 96 (:1003).  I: 4 columns, the
  * contravariant I^mu per particle (for instance the j^mu of ccake_smear_sources; I[3] is ignored when dim == 2); Iq: 3

@@ -30,7 +30,7 @@ RATE = 64
 HOST, DEVICE = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ERANGE = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_invert_forward_table", "ccake_smear_sources",
+EXPORTS = ["ccake_create", "ccake_destroy", "ccake_load_particles", "ccake_load_eos_table", "ccake_invert_eos_table", "ccake_invert_forward_table", "ccake_smear_sources", "ccake_smear_sources_noalloc",
            "ccake_set_sources",
            "ccake_slab_load", "ccake_slab_export_halo", "ccake_slab_import_ghosts", "ccake_slab_substep", "ccake_slab_substep_part", "ccake_slab_export_records", "ccake_slab_import_records",
            "ccake_slab_export_migrants", "ccake_slab_import_migrants", "ccake_slab_commit", "ccake_slab_info", "ccake_slab_gids",
@@ -80,6 +80,7 @@ def lib():
         L.ccake_invert_forward_table.argtypes = [vp, C.POINTER(i32), C.POINTER(vp), vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(vp), i32,
                                                  C.POINTER(i32), vp, vp, C.POINTER(i64), i32]
         L.ccake_smear_sources.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp), i32]
+        L.ccake_smear_sources_noalloc.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), vp, C.c_double, C.c_double, C.POINTER(vp)]
         L.ccake_set_sources.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), i32]
         L.ccake_slab_load.argtypes = [vp, i64, i64, i32, C.POINTER(i32), C.POINTER(vp), vp, i32, C.c_double, C.c_double, C.c_double, i32]
         L.ccake_slab_export_halo.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64)]
@@ -268,6 +269,16 @@ class Ccake:
         self._chk(lib().ccake_smear_sources(self._h, t.size, pp, rr, t.ctypes.data, float(h_source), float(eta_norm),
                                             oo, HOST), "ccake_smear_sources")
         return out
+
+    def smear_sources_noalloc(self, p, r, t, h_source, eta_norm, out):
+        """ccake_smear_sources_noalloc: p (4), r (3) lists of CUDA tensors of npartons doubles, t a CUDA tensor, out a list of 4
+        CUDA tensors of n doubles (overwritten).  Asynchronous: valid after synchronize().  Allocates nothing."""
+        assert all(_is_torch(x) and x.is_cuda for x in list(p) + list(r) + [t] + list(out))
+        pp = (C.c_void_p * 4)(*[x.data_ptr() for x in p])
+        rr = (C.c_void_p * 3)(*[x.data_ptr() for x in r])
+        oo = (C.c_void_p * 4)(*[x.data_ptr() for x in out])
+        self._chk(lib().ccake_smear_sources_noalloc(self._h, int(t.numel()), pp, rr, t.data_ptr(), float(h_source),
+                                                    float(eta_norm), oo), "ccake_smear_sources_noalloc")
 
     def set_sources(self, I=None, Iq=None):
         """ccake_set_sources (Eq. 38): I [4, n] contravariant I^mu, Iq [3, n] (numpy host arrays, or lists of

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -498,6 +499,92 @@ smear_sources_kernel(int64_t n, int64_t npad, const double* __restrict__ Y, cons
     const int64_t o = orig[i];
     for (int m = 0; m < 4; ++m) out[m * n + o] = pref * acc[m];
   }
+}
+
+/* ---- ccake_smear_sources_noalloc: the same smearing without any allocation (include/ccake.h) ----
+   The packed parton array that ccake_smear_sources keeps in a cudaMalloc'ed buffer lives here in a file-scope device array of
+   8 x CCAKE_SMEAR_NOALLOC_MAX doubles (1 MiB, held by every GPU that loads the library until the process exits).  Row m of the
+   array starts at m * CCAKE_SMEAR_NOALLOC_MAX: rows 0..3 = p^mu, 4..6 = r.  Every call overwrites entries [0, npartons) of every
+   row it reads and reads nothing else, so nothing has to start at zero; the array is SHARED by all calls (all contexts, all
+   streams of a device): calls that overlap on the GPU race.
+   In host code the NAME g_smear_scratch is a host-side stand-in, not a device address: the host obtains the address once per
+   device with cudaGetSymbolAddress (smear_scratch_address) and hands that pointer to the kernels. */
+static __device__ __align__(256) double g_smear_scratch[8 * CCAKE_SMEAR_NOALLOC_MAX];
+
+struct SmearCols { const double* p[4]; const double* r[3]; const double* t; };
+
+/* partons -> scratch, already in the form the tiles want: a parton outside the time window x0 - dx0 < t <= x0 gets zero
+   momentum and a position that fails the cut-off test (what smear_sources_kernel does while staging a tile) */
+__global__ void smear_pack_kernel(SmearCols in, int64_t np_, double x0, double dx0, double* __restrict__ scratch) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= np_) return;
+  const double tk = in.t[k];
+  const bool ok = tk > x0 - dx0 && tk <= x0;
+  for (int m = 0; m < 4; ++m) scratch[(int64_t)m * CCAKE_SMEAR_NOALLOC_MAX + k] = ok ? in.p[m][k] : 0.0;
+  for (int a = 0; a < 3; ++a) scratch[(int64_t)(4 + a) * CCAKE_SMEAR_NOALLOC_MAX + k] = ok ? in.r[a][k] : 1.0e150;
+}
+
+/* smear_sources_kernel with the partons read from the scratch array and the four components written straight into the
+   caller's columns (original particle order); same arithmetic in the same order */
+struct SmearOut { double* j[4]; };
+template <int D>
+__global__ void __launch_bounds__(SRC_TILE)
+smear_sources_scratch_kernel(int64_t n, int64_t npad, const double* __restrict__ Y, const uint32_t* __restrict__ orig, int64_t np_,
+                             const double* __restrict__ scratch, double pref, double hs, double sig_d, SmearOut out) {
+  __shared__ double sp[4][SRC_TILE], sr[3][SRC_TILE];
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  const int64_t ic = (i < n) ? i : n - 1;
+  double xa[3] = {0.0, 0.0, 0.0};
+  for (int k = 0; k < D; ++k) xa[k] = Y[(CCAKE_R1 + k) * npad + ic];
+  const double inv_h = 1.0 / hs, cut2 = (2.0 * hs) * (2.0 * hs);
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int64_t base = 0; base < np_; base += SRC_TILE) {
+    const int64_t k = base + threadIdx.x;
+    __syncthreads();
+    {
+      const bool in = k < np_;
+      for (int m = 0; m < 4; ++m) sp[m][threadIdx.x] = in ? scratch[(int64_t)m * CCAKE_SMEAR_NOALLOC_MAX + k] : 0.0;
+      for (int a = 0; a < 3; ++a) sr[a][threadIdx.x] = in ? scratch[(int64_t)(4 + a) * CCAKE_SMEAR_NOALLOC_MAX + k] : 1.0e150;
+    }
+    __syncthreads();
+    const int cnt = (int)min((int64_t)SRC_TILE, np_ - base);
+    for (int b = 0; b < cnt; ++b) {
+      double r2 = 0.0;
+#pragma unroll
+      for (int a = 0; a < D; ++a) { const double dr = xa[a] - sr[a][b]; r2 += dr * dr; }
+      if (r2 < cut2) {
+        const double q = sqrt(r2) * inv_h, t = 2.0 - q;
+        const double W = sig_d * ((q <= 1.0) ? fma(q * q, fma(0.75, q, -1.5), 1.0) : 0.25 * t * t * t);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) acc[m] = fma(sp[m][b], W, acc[m]);
+      }
+    }
+  }
+  if (i < n) {
+    const int64_t o = orig[i];
+    for (int m = 0; m < 4; ++m) out.j[m][o] = pref * acc[m];
+  }
+}
+
+/* device address of g_smear_scratch on the CURRENT device (one copy of the array per device): looked up once per device */
+int smear_scratch_address(ccake_ctx* c, double** out) {
+  constexpr int MAXDEV = 64;
+  static std::mutex mu;
+  static double* addr[MAXDEV] = {nullptr};
+  if (c->device < 0 || c->device >= MAXDEV) { c->err = "device ordinal beyond the scratch table"; return CCAKE_EINVAL; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[c->device]) {
+    double* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_smear_scratch);     /* the device of the context is current */
+    if (e != cudaSuccess || !ptr) {
+      c->err = std::string("cudaGetSymbolAddress(g_smear_scratch): ") + cudaGetErrorString(e);
+      cudaGetLastError();
+      return CCAKE_ECUDA;
+    }
+    addr[c->device] = ptr;
+  }
+  *out = addr[c->device];
+  return CCAKE_OK;
 }
 
 int refresh(ccake_ctx* c) {
@@ -1171,6 +1258,49 @@ int ccake_smear_sources(ccake_ctx* c, int64_t npartons, const double* const p[4]
   cudaFree(dsrc);
   cudaFree(dout);
   return rc;
+}
+
+int ccake_smear_sources_noalloc(ccake_ctx* c, int64_t npartons, const double* const p[4], const double* const r[3],
+                                const double* t, double h_source, double eta_norm, double* const j[4]) {
+  if (!c) return CCAKE_EINVAL;
+  if (npartons < 0 || !p || !r || (npartons > 0 && !t) || !j || !(h_source > 0.0)) {
+    c->err = "bad arguments to ccake_smear_sources_noalloc";
+    return CCAKE_EINVAL;
+  }
+  if (npartons > CCAKE_SMEAR_NOALLOC_MAX) {
+    c->err = "ccake_smear_sources_noalloc: npartons = " + std::to_string(npartons) + " exceeds CCAKE_SMEAR_NOALLOC_MAX = " +
+             std::to_string((long long)CCAKE_SMEAR_NOALLOC_MAX) + " (the fixed scratch array); use ccake_smear_sources";
+    return CCAKE_EINVAL;
+  }
+  for (int m = 0; m < 4; ++m) if ((npartons > 0 && !p[m]) || !j[m]) { c->err = "null column"; return CCAKE_EINVAL; }
+  for (int a = 0; a < 3; ++a) if (npartons > 0 && !r[a]) { c->err = "null column"; return CCAKE_EINVAL; }
+  if (!c->loaded) { c->err = "smear before load"; return CCAKE_ESTATE; }
+  CK(cudaSetDevice(c->device));
+  double* scratch = nullptr;
+  if (int rc = smear_scratch_address(c, &scratch)) return rc;
+  const int64_t N = c->N, np = c->npad, ns = npartons;
+  cudaStream_t st = c->stream;
+  const Geom gm = make_geom(c->P.coords, c->x0);
+  const double pi = 3.14159265358979323846;
+  const int D = c->P.dim;
+  const double sig_d = (D == 2) ? 10.0 / (7.0 * pi * h_source * h_source) : 1.0 / (pi * h_source * h_source * h_source);
+  const double pref = eta_norm / (c->P.dx0 * gm.sqrtg);
+  if (ns > 0) {
+    SmearCols in;
+    for (int m = 0; m < 4; ++m) in.p[m] = p[m];
+    for (int a = 0; a < 3; ++a) in.r[a] = r[a];
+    in.t = t;
+    smear_pack_kernel<<<nblk(ns, 256), 256, 0, st>>>(in, ns, c->x0, c->P.dx0, scratch);
+    c->launches += 1;
+  }
+  SmearOut out;
+  for (int m = 0; m < 4; ++m) out.j[m] = j[m];
+  if (D == 2)
+    smear_sources_scratch_kernel<2><<<nblk(N, SRC_TILE), SRC_TILE, 0, st>>>(N, np, c->Y[0], c->orig[0], ns, scratch, pref, h_source, sig_d, out);
+  else
+    smear_sources_scratch_kernel<3><<<nblk(N, SRC_TILE), SRC_TILE, 0, st>>>(N, np, c->Y[0], c->orig[0], ns, scratch, pref, h_source, sig_d, out);
+  c->launches += 1;
+  return launch_check(c, "smear_sources_scratch_kernel");
 }
 
 int ccake_set_sources(ccake_ctx* c, const double* const I[4], const double* const Iq[3], int32_t memspace) {
