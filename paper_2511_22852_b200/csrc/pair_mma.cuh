@@ -44,6 +44,9 @@
 
 namespace ccake {
 
+#ifndef CCAKE_CL_LBK
+#define CCAKE_CL_LBK 4                       /* candidates a thread of cand_list_kernel tests per step */
+#endif
 #ifndef CCAKE_PM_WARPS
 #define CCAKE_PM_WARPS 16
 #endif
@@ -404,7 +407,7 @@ template <class Op> struct PairCfg {
 template <int D>
 __global__ void __launch_bounds__(BH)
 cand_list_kernel(int64_t n, const Grid* __restrict__ grid, Sorted so) {
-  constexpr int NW = BH / 32, LBK = 4;
+  constexpr int NW = BH / 32, LBK = CCAKE_CL_LBK;
   __shared__ float s_lo[NW][3], s_hi[NW][3];
   __shared__ int wcnt[LBK * NW];
   __shared__ uint32_t rb0[MAXROW], rcum[MAXROW + 1];
@@ -457,6 +460,10 @@ cand_list_kernel(int64_t n, const Grid* __restrict__ grid, Sorted so) {
     }
     __syncthreads();
     const uint32_t raw = rcum[nr];
+    int rowh[LBK];                                   /* row of the thread's previous entry: f only grows, and a row holds
+                                                        hundreds of entries, so the search is a step or two from there */
+#pragma unroll
+    for (int u = 0; u < LBK; ++u) rowh[u] = 0;
 #pragma unroll 1
     for (uint32_t fb = 0; fb < raw; fb += LBK * BH) {
       bool r[LBK];
@@ -467,12 +474,9 @@ cand_list_kernel(int64_t n, const Grid* __restrict__ grid, Sorted so) {
         r[u] = false;
         j[u] = 0;
         if (f < raw) {
-          int row = 0;
-#pragma unroll
-          for (int st = MAXROW / 2; st > 0; st >>= 1) {                     /* rcum is monotone: binary search */
-            const int rq = row + st;
-            if (rq < nr && rcum[rq] <= f) row = rq;
-          }
+          int row = rowh[u];                          /* the last row with rcum[row] <= f (rcum is monotone) */
+          while (row + 1 < nr && rcum[row + 1] <= f) ++row;
+          rowh[u] = row;
           j[u] = rb0[row] + (f - rcum[row]);
           r[u] = box_dist2<D>(xf[j[u]], blo, bhi) <= cutm2;
         }
