@@ -44,6 +44,9 @@
 
 namespace ccake {
 
+#ifndef CCAKE_PM_CARRY
+#define CCAKE_PM_CARRY 1                     /* passes that read cached masks carry the < 4 left-over candidates of a tile over */
+#endif
 #ifndef CCAKE_CL_LBK
 #define CCAKE_CL_LBK 4                       /* candidates a thread of cand_list_kernel tests per step */
 #endif
@@ -175,7 +178,7 @@ template <int D_, bool HASH_ = false>
 struct SmoothOp {
   static constexpr int D = D_;
   static constexpr bool HASH = HASH_;
-  static constexpr bool COUNT = true, GIDMAJOR = false;
+  static constexpr bool COUNT = true, GIDMAJOR = false, CARRY = false;
   static constexpr int NREC = 8, NJ = 1, NT = 1, oM = 3, XO = 0, NSLOT = NSLOT_S;
   static constexpr int elem(int, int, int n) { return (n <= 4) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
@@ -271,7 +274,7 @@ __device__ __forceinline__ void write_grad_record(double* __restrict__ rg, const
 template <int D_, bool VISC, bool DIFF>
 struct GradOp {
   static constexpr int D = D_;
-  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = true;
+  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = true, CARRY = CCAKE_PM_CARRY != 0;
   static constexpr int eM = make_glayout(D_, VISC, DIFF).M, eP = make_glayout(D_, VISC, DIFF).P, eU = make_glayout(D_, VISC, DIFF).U,
                        eV = make_glayout(D_, VISC, DIFF).V, eB = make_glayout(D_, VISC, DIFF).B, eK = make_glayout(D_, VISC, DIFF).K,
                        eAL = make_glayout(D_, VISC, DIFF).AL;
@@ -359,7 +362,7 @@ struct GradOp {
 template <int D_>
 struct EpsGradOp {
   static constexpr int D = D_;
-  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = false;
+  static constexpr bool HASH = false, COUNT = false, GIDMAJOR = false, CARRY = CCAKE_PM_CARRY != 0;
   static constexpr int NREC = 8, NJ = D, NT = 1, oM = 3, XO = 0, NSLOT = NSLOT_G;
   static constexpr int elem(int, int, int n) { return (n <= 1) ? 3 + n : ELEM_NONE; }
   __device__ static __forceinline__ void weights(const KParams& kp, const PairGeom<D>& g, double (&aw)[NJ]) {
@@ -378,20 +381,23 @@ struct EpsGradOp {
 };
 
 /* ------------------------------------------------------------------------------------ shared memory ---- */
-/* Tile: unit c (16 bytes = 2 doubles) of staged candidate k sits at unit index c * CSTRIDE + k with CSTRIDE =
-   TILE_B + 1, so its 16-byte bank group is (c + k) mod 8: the staging writes (consecutive c, same k) are
+/* Tile: unit c (16 bytes = 2 doubles) of staged candidate k sits at unit index c * CSTRIDE + k with CSTRIDE = 1 mod 8
+   (TILE_B + 1, plus the carry columns of the passes that have them), so its 16-byte bank group is (c + k) mod 8: the staging writes (consecutive c, same k) are
    conflict-free and the 8-byte operand reads of a quad (8 columns x 4 candidates) spread over the bank groups. */
 template <class Op> struct PairCfg {
   static constexpr int NR = Op::NREC;
   static constexpr int NU = NR / 2;
   static constexpr int NSLOT = Op::NSLOT, TILE_B = NSLOT * HALF_B;
-  static constexpr int CSTRIDE = TILE_B + 1;
+  static constexpr int NCARRY = Op::CARRY ? 3 * NGRP : 0;   /* carry columns behind the ring: 3 per group (a multiple of 8) */
+  static constexpr int CARRY0 = TILE_B + 1;                 /* first carry column */
+  static constexpr int CSTRIDE = TILE_B + 1 + NCARRY;
+  static constexpr int FSTRIDE = HALF_B + 4;                /* FIFO entries per group: a tile and up to 3 carried candidates */
   static constexpr int NSUM = 8 * Op::NT * Op::NJ;          /* sums per home particle */
   static constexpr int SSTRIDE = NSUM + 2;                  /* scratch row of a home in the epilogue (even, skewed) */
   static constexpr size_t B_PAY = sizeof(double2) * NU * CSTRIDE;
   static constexpr size_t B_PAYX = sizeof(float4) * TILE_B;
   static constexpr size_t B_LIST = sizeof(uint32_t) * (LCAP + LB * PT);
-  static constexpr size_t B_FIFO = sizeof(uint16_t) * NGRP * HALF_B;   /* tile entries waiting per group */
+  static constexpr size_t B_FIFO = sizeof(uint16_t) * NGRP * FSTRIDE;  /* tile entries waiting per group */
   static constexpr size_t B_MASK = sizeof(uint4) * NSLOT * NGRP;
   static constexpr size_t B_RING = B_PAY + B_PAYX + B_LIST + B_FIFO + B_MASK;
   static constexpr size_t B_SCRATCH = sizeof(double) * BH * SSTRIDE;
@@ -532,8 +538,8 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   double2* pay = reinterpret_cast<double2*>(smem_raw);                  /* [NU][CSTRIDE] staged records        */
   float4* payx = reinterpret_cast<float4*>(pay + NU * CSTRIDE);         /* [TILE_B] FP32 positions of the tile */
   uint32_t* list = reinterpret_cast<uint32_t*>(payx + TILE_B);          /* [LCAP + LB * PT] block candidate list */
-  uint16_t* fifo = reinterpret_cast<uint16_t*>(list + LCAP + LB * PT);  /* [NGRP][HALF_B] byte offsets of the staged entries that passed, per group */
-  uint4* mstage = reinterpret_cast<uint4*>(fifo + NGRP * HALF_B);       /* [NSLOT][NGRP] cached hit masks of the staged tiles (MC == 2) */
+  uint16_t* fifo = reinterpret_cast<uint16_t*>(list + LCAP + LB * PT);  /* [NGRP][FSTRIDE] byte offsets of the staged entries that passed, per group */
+  uint4* mstage = reinterpret_cast<uint4*>(fifo + NGRP * PairCfg<Op>::FSTRIDE);       /* [NSLOT][NGRP] cached hit masks of the staged tiles (MC == 2) */
   __shared__ float s_lo[NW][3], s_hi[NW][3];
   __shared__ int wcnt[LB * NW];
   __shared__ uint32_t rb0[MAXROW], rcum[MAXROW + 1];
@@ -740,6 +746,14 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
   auto flush = [&](const int cnt) {
     const int ntile = (cnt + HALF_B - 1) / HALF_B;
     const int tt0 = tt;
+    /* CARRY: the tl & 3 candidates of a tile that do not fill a quad are not evaluated as a partial quad (a whole quad's cost
+       for 2.5 candidates on average, once per tile and group); their records are copied into the group's 3 carry columns
+       behind the ring and lead the FIFO of the next tile.  Only the last tile of a flush ends with a partial quad.  (Not in
+       the smoothing pass: its union masks are per tile.) */
+    constexpr bool CARRY = Op::CARRY && MC == 2;
+    int ncarry[GPW];
+#pragma unroll
+    for (int gg = 0; gg < GPW; ++gg) ncarry[gg] = 0;
     int ni = 0;                                                   /* next tile of this flush the warp has to issue */
     uint32_t jn = load_j(cnt, ntile, 0);
     auto try_issue = [&](const int upto, const bool block) {
@@ -771,7 +785,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
       const bool cached = (MC != 0) && tt < mtiles;
 #pragma unroll
       for (int gg = 0; gg < GPW; ++gg) {
-        uint16_t* ff = fifo + (w * GPW + gg) * HALF_B;
+        uint16_t* ff = fifo + (w * GPW + gg) * PairCfg<Op>::FSTRIDE;
         /* survivors of the tile for this group: the cached exact-union mask, or the FP32 test against the group box */
         uint32_t bal[NR32];
         if (MC == 2 && cached) {
@@ -792,7 +806,7 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
           }
         }
         /* compaction, ascending: entry k of the tile goes to position pos[r] */
-        int pos[NR32], tl = 0;
+        int pos[NR32], tl = CARRY ? ncarry[gg] : 0;               /* the carried candidates are ff[0 .. ncarry) already */
 #pragma unroll
         for (int r = 0; r < NR32; ++r) {
           pos[r] = tl + __popc(bal[r] & lt_mask);
@@ -816,7 +830,33 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
 #pragma unroll 1
           for (const uint16_t* fp = fq; fp != fend; fp += 4) quad(gg, *fp, true);
         }
-        if (tl & 3) {
+        if (CARRY && t + 1 < ntile) {
+          const int rem = tl & 3;
+          if (rem) {
+            /* left-over i (FIFO entry 4 nfull + i) -> carry column i of this group: NU units each, all read before any is
+               written (with nfull == 0 an entry may already sit in its carry column) */
+            constexpr int NCP = (3 * NU + 31) / 32;
+            const uint32_t cbase = (uint32_t)(PairCfg<Op>::CARRY0 + (w * GPW + gg) * 3) * 16u;
+            double2 cv[NCP];
+            uint32_t cdst[NCP];
+#pragma unroll
+            for (int x = 0; x < NCP; ++x) {
+              const int idx = x * 32 + lane, ci = idx / NU, cu = idx - ci * NU;
+              cdst[x] = 0xffffffffu;
+              if (ci < rem) {
+                const uint32_t so_ = ff[4 * nfull + ci];
+                cv[x] = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(pay) + (size_t)cu * CSTRIDE * 16 + so_);
+                cdst[x] = (uint32_t)cu * CSTRIDE * 16u + cbase + (uint32_t)ci * 16u;
+              }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int x = 0; x < NCP; ++x)
+              if (cdst[x] != 0xffffffffu) *reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(pay) + cdst[x]) = cv[x];
+            if (lane < rem) ff[lane] = (uint16_t)(cbase + (uint32_t)lane * 16u);
+          }
+          ncarry[gg] = rem;
+        } else if (tl & 3) {
           const bool act = 4 * nfull + tig < tl;
           const uint32_t nib = quad(gg, ff[act ? 4 * nfull + tig : 4 * nfull], act);
           if (MC == 1) nibs = (lane == nfull) ? nib : nibs;
