@@ -833,26 +833,20 @@ pair_mma_kernel(int64_t n, KParams kp, const Grid* __restrict__ grid, Sorted so,
         if (CARRY && t + 1 < ntile) {
           const int rem = tl & 3;
           if (rem) {
-            /* left-over i (FIFO entry 4 nfull + i) -> carry column i of this group: NU units each, all read before any is
-               written (with nfull == 0 an entry may already sit in its carry column) */
+            /* left-over i (FIFO entry 4 nfull + i) -> carry column i of this group, NU units each.  With nfull == 0 the
+               first ncarry entries are carried ones and sit in their columns already; all others come from the ring. */
             constexpr int NCP = (3 * NU + 31) / 32;
             const uint32_t cbase = (uint32_t)(PairCfg<Op>::CARRY0 + (w * GPW + gg) * 3) * 16u;
-            double2 cv[NCP];
-            uint32_t cdst[NCP];
+            const int ci0 = (nfull == 0) ? ncarry[gg] : 0;
 #pragma unroll
             for (int x = 0; x < NCP; ++x) {
               const int idx = x * 32 + lane, ci = idx / NU, cu = idx - ci * NU;
-              cdst[x] = 0xffffffffu;
-              if (ci < rem) {
-                const uint32_t so_ = ff[4 * nfull + ci];
-                cv[x] = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(pay) + (size_t)cu * CSTRIDE * 16 + so_);
-                cdst[x] = (uint32_t)cu * CSTRIDE * 16u + cbase + (uint32_t)ci * 16u;
+              if (ci >= ci0 && ci < rem) {
+                unsigned char* col = reinterpret_cast<unsigned char*>(pay) + (size_t)cu * CSTRIDE * 16;
+                *reinterpret_cast<double2*>(col + cbase + (uint32_t)ci * 16u) = *reinterpret_cast<const double2*>(col + ff[4 * nfull + ci]);
               }
             }
             __syncwarp();
-#pragma unroll
-            for (int x = 0; x < NCP; ++x)
-              if (cdst[x] != 0xffffffffu) *reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(pay) + cdst[x]) = cv[x];
             if (lane < rem) ff[lane] = (uint16_t)(cbase + (uint32_t)lane * 16u);
           }
           ncarry[gg] = rem;
