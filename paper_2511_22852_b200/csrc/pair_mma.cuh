@@ -26,9 +26,10 @@
  *     payload records are copied with cp.async, HALF_B at a time and taken with a stride through the list, into a
  *     ring of NSLOT tiles (3 in the gradient pass, 6 in the smoothing pass) in shared memory (component-major, one-unit skew) whose arrival is tracked by one
  *     mbarrier per slot; there is no block barrier per tile.
- *   - Per tile and group the warp tests the 128 candidates against the FP32 box of the group's 8 homes (4 per lane,
- *     ballots) and compacts the survivors into a FIFO of slot numbers; quads of 4 candidates are taken from it,
- *     leftovers (< 4) wait for the next tile (the ring keeps the previous tile resident for exactly that).
+ *   - Per tile and group the warp tests the HALF_B candidates against the FP32 box of the group's 8 homes (ballots)
+ *     and compacts the survivors into a FIFO of byte offsets; quads of 4 candidates are taken from it.  Leftovers (< 4)
+ *     form a partial quad (smoothing pass) or are copied into carry columns behind the ring and lead the next tile's
+ *     FIFO (passes that read cached masks).
  *   - The neighbour decision is the exact FP64 test r2 = (dx*dx + dy*dy) + dz*dz < (2h)^2 with round-to-nearest
  *     multiplies and adds and no FMA contraction (DESIGN reading 8), per pair; a miss enters the MMA with weight
  *     exactly 0.  The smoothing pass records which candidates hit at least one home of the group and stores that
