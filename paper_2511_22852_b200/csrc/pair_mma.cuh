@@ -24,7 +24,7 @@
  *   - Candidates of a block come from cand_list_kernel (once per substep, global memory, both passes) or, for a
  *     block whose list does not fit there, from a list built inside the pass (interleaved sweeps).  Their AoS
  *     payload records are copied with cp.async, HALF_B at a time and taken with a stride through the list, into a
- *     ring of NSLOT tiles (3 in the gradient pass, 6 in the smoothing pass) in shared memory (component-major, one-unit skew) whose arrival is tracked by one
+ *     ring of NSLOT tiles (2 in the gradient pass, 6 in the smoothing pass) in shared memory (component-major, one-unit skew) whose arrival is tracked by one
  *     mbarrier per slot; there is no block barrier per tile.
  *   - Per tile and group the warp tests the HALF_B candidates against the FP32 box of the group's 8 homes (ballots)
  *     and compacts the survivors into a FIFO of byte offsets; quads of 4 candidates are taken from it.  Leftovers (< 4)
@@ -63,7 +63,7 @@ constexpr int PT = 32 * PM_WARPS;            /* threads per block               
 constexpr int NGRP = PM_WARPS * PM_GPW;      /* groups per block                                 */
 constexpr int BH = 8 * NGRP;                 /* home particles per block                         */
 #ifndef CCAKE_PM_TILE
-#define CCAKE_PM_TILE 96
+#define CCAKE_PM_TILE 128
 #endif
 #ifndef CCAKE_PM_MINB
 #define CCAKE_PM_MINB 2
@@ -72,10 +72,10 @@ constexpr int HALF_B = CCAKE_PM_TILE;        /* candidates per tile (a multiple 
 constexpr int PM_MINB = CCAKE_PM_MINB;       /* resident blocks per SM the register budget is set for */
 constexpr int NR32 = HALF_B / 32;            /* candidates a lane tests per tile and group       */
 #ifndef CCAKE_PM_NSLOT
-#define CCAKE_PM_NSLOT 3
+#define CCAKE_PM_NSLOT 2
 #endif
 #ifndef CCAKE_PM_NSLOT_S
-#define CCAKE_PM_NSLOT_S 6                   /* measured on C4: 3 / 4 / 5 / 6 / 8 slots -> 8.32 / 8.37 / 8.25 / 8.21 / 8.27 ms */
+#define CCAKE_PM_NSLOT_S 6                   /* measured on C4 with tiles of 128: 4 / 5 / 6 / 7 / 8 slots -> 7.81 / 7.66 / 7.64 / 7.65 / 7.76 ms */
 #endif
 constexpr int NSLOT_G = CCAKE_PM_NSLOT;      /* tiles resident in shared memory: the current one and those in flight (Op::NSLOT) */
 constexpr int NSLOT_S = CCAKE_PM_NSLOT_S;    /* ... of the smoothing pass, whose records are a quarter of the gradient pass's */
