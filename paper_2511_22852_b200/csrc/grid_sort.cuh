@@ -383,12 +383,11 @@ __global__ void pack_smoothing_kernel(const double* __restrict__ Y, int64_t npad
   so.x[0][i] = x; so.x[1][i] = y; so.x[2][i] = z;
   so.xf[i] = make_float4((float)(x - grid->xmin[0]), (float)(y - grid->xmin[1]), (D == 3) ? (float)(z - grid->xmin[2]) : 0.f,
                          __uint_as_float((uint32_t)i));   /* w: the sorted slot (read by the neighbour-hash test pass) */
-  double2* r = reinterpret_cast<double2*>(so.rec_s + i * 8);
-  r[0] = make_double2(x, y);
   const double m = Y[CCAKE_MASS * npad + a];              /* payload columns carry the SPH weight m_b (pair_mma.cuh) */
-  r[1] = make_double2(z, m);
-  r[2] = make_double2(m * Y[CCAKE_S * npad + a], m * Y[CCAKE_NB * npad + a]);
-  r[3] = make_double2(m * Y[CCAKE_NS * npad + a], m * Y[CCAKE_NQ * npad + a]);
+  double* r = so.rec_s + i * 8;                           /* 64-byte record: two 32-byte stores (STG.256) */
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(r), "d"(x), "d"(y), "d"(z), "d"(m) : "memory");
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(r + 4), "d"(m * Y[CCAKE_S * npad + a]), "d"(m * Y[CCAKE_NB * npad + a]),
+               "d"(m * Y[CCAKE_NS * npad + a]), "d"(m * Y[CCAKE_NQ * npad + a]) : "memory");
 }
 
 }  // namespace ccake

@@ -256,9 +256,20 @@ __host__ __device__ constexpr int grad_pos(int D, bool visc, bool diff, int e) {
       if (grad_slot_elem(D, visc, diff, n, s) == e) return GREC_B0 + 4 * n + s;
   return -1;
 }
-/* thermo kernel: scatter the elements el[0 .. L.N) of one particle into its record */
+/* 32-byte global store / load (sm_100: STG.256 / LDG.256); the address is 32-byte aligned */
+__device__ __forceinline__ void st_global_v4(double* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+__device__ __forceinline__ void ldg_nc_v4(const double* p, double& a, double& b, double& c, double& d) {
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+#ifndef CCAKE_V4
+#define CCAKE_V4 1
+#endif
+/* thermo kernel: scatter the elements el[0 .. L.N) of one particle into its record; pos: the position, which sits in the
+   free slots 1..3 of block 7 */
 template <int D, bool VISC, bool DIFF>
-__device__ __forceinline__ void write_grad_record(double* __restrict__ rg, const double* el) {
+__device__ __forceinline__ void write_grad_record(double* __restrict__ rg, const double* el, const double (&pos)[3]) {
 #pragma unroll
   for (int n = 0; n < 8; ++n) {
     double v[4];
@@ -266,9 +277,14 @@ __device__ __forceinline__ void write_grad_record(double* __restrict__ rg, const
     for (int s = 0; s < 4; ++s) {
       const int e = grad_slot_elem(D, VISC, DIFF, n, s);
       v[s] = (e >= 0) ? el[e] : 0.0;
+      if (4 * n + s >= GREC_X) v[s] = pos[4 * n + s - GREC_X];
     }
+#if CCAKE_V4
+    st_global_v4(rg + GREC_B0 + 4 * n, v[0], v[1], v[2], v[3]);
+#else
     reinterpret_cast<double2*>(rg + GREC_B0 + 4 * n)[0] = make_double2(v[0], v[1]);
     reinterpret_cast<double2*>(rg + GREC_B0 + 4 * n)[1] = make_double2(v[2], v[3]);
+#endif
   }
 }
 

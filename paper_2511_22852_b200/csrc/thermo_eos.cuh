@@ -70,12 +70,24 @@ __device__ inline ThermoOut eos_table_lookup(const TableDev& tb, double s, const
         const int64_t node = (((int64_t)(i0[0] + b0) * tb.dims[1] + (i0[1] + b1)) * tb.dims[2] + (i0[2] + b2)) * tb.dims[3] + i0[3];
         const double2* __restrict__ p0 = reinterpret_cast<const double2*>(tb.data + node * TB_STRIDE);
         const double wl = w012 * (1.0 - t[3]), wh = w012 * t[3];
+#if CCAKE_V4
+        static_assert(TB_STRIDE % 4 == 0, "32-byte loads");
+#pragma unroll
+        for (int u = 0; u < TB_STRIDE / 4; ++u) {
+          double lo[4], hi[4];
+          ldg_nc_v4(reinterpret_cast<const double*>(p0) + 4 * u, lo[0], lo[1], lo[2], lo[3]);
+          ldg_nc_v4(reinterpret_cast<const double*>(p0) + TB_STRIDE + 4 * u, hi[0], hi[1], hi[2], hi[3]);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) { out[4 * u + c] += wl * lo[c]; out[4 * u + c] += wh * hi[c]; }
+        }
+#else
 #pragma unroll
         for (int u = 0; u < TB_STRIDE / 2; ++u) {
           const double2 lo = __ldg(p0 + u), hi = __ldg(p0 + TB_STRIDE / 2 + u);
           out[2 * u] += wl * lo.x; out[2 * u] += wh * hi.x;
           out[2 * u + 1] += wl * lo.y; out[2 * u + 1] += wh * hi.y;
         }
+#endif
       }
   th.T = out[CCAKE_COL_T];
   for (int q = 0; q < NQ; ++q) { th.mu[q] = out[CCAKE_COL_MUB + q]; th.wq[q] = out[CCAKE_COL_WB + q]; }
@@ -551,8 +563,8 @@ thermo_kernel(int64_t n, KParams kp, const double* __restrict__ x0_dev, double x
     }
   }
   double* __restrict__ rg = so.rec_g + i * GREC_D;
-  write_grad_record<TD, TV, TF>(rg, el);
-  rg[GREC_X] = so.x[0][i]; rg[GREC_X + 1] = so.x[1][i]; rg[GREC_X + 2] = so.x[2][i];      /* the free slots of block 7 */
+  const double xyz[3] = {so.x[0][i], so.x[1][i], so.x[2][i]};
+  write_grad_record<TD, TV, TF>(rg, el, xyz);                /* the position goes into the free slots of block 7 */
 }
 
 }  // namespace ccake
